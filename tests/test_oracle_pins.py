@@ -1,0 +1,488 @@
+"""Pins for the CPU oracle (oracle/dns_oracle.py): it is checked against what the paper and the mathematics
+fix -- closed forms, invariants, an independent eigen-solve, a published eigenvalue, brute force -- never
+against itself.  Pin numbers P1..P14 follow SURVEY.md section 8(c).  All tests run on CPU (`-m "not gpu"`).
+"""
+import os
+
+import numpy as np
+import pytest
+import scipy.linalg as sla
+from numpy.polynomial import chebyshev as C
+from numpy.polynomial import polynomial as npoly
+
+from oracle.dns_oracle import (COUETTE, POISEUILLE_CMF, Oracle, cheb_D, cheb_points, clamped_D4,
+                               clenshaw_curtis, dft_matrix)
+from paper_2306_12739_b200 import inputs
+
+PI = np.pi
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def small_cfg(flow=COUETTE, Nx=12, Ny=25, Nz=12, E=2, Re=400.0, dt=0.02, rms=0.05, cid=1, box=2):
+    return inputs.Config(cid, flow, Re, 1.75 * PI, 1.2 * PI, Nx, Ny, Nz, E, dt, 1, rms, 0, box=box)
+
+
+def make(cfg, zero_pert=False, members=None):
+    o = Oracle(*inputs.plan_args(cfg, E=None if members is None else len(members)))
+    st = inputs.make_state(cfg, members)
+    s = 0.0 if zero_pert else 1.0
+    o.set_state(s * st["vhat"], s * st["etahat"], st["U00"], st["W00"])
+    return o, st
+
+
+# ------------------------------------------------------------------------------------------------ P1
+@pytest.mark.parametrize("Ny", [9, 33, 65])
+def test_P1_cheb_D_exact_on_polynomials(Ny):
+    y = cheb_points(Ny)
+    assert np.all(np.diff(y) > 0) and y[0] == -1.0 and abs(y[-1] - 1.0) < 1e-15
+    D = cheb_D(Ny)
+    assert np.abs(D @ np.ones(Ny)).max() < 1e-11 * Ny ** 2
+    for k in range(1, Ny):
+        err = np.abs(D @ y ** k - k * y ** (k - 1)).max()
+        assert err < 1e-11 * Ny ** 2, (k, err)
+
+
+@pytest.mark.parametrize("Ny", [8, 9, 33, 97])
+def test_clenshaw_curtis_exact(Ny):
+    y, w = cheb_points(Ny), clenshaw_curtis(Ny)
+    assert abs(w.sum() - 2.0) < 1e-13
+    for k in range(Ny):
+        exact = 0.0 if k % 2 else 2.0 / (k + 1)
+        assert abs(w @ y ** k - exact) < 1e-12
+
+
+# ------------------------------------------------------------------------------------------------ P2
+def test_P2_laminar_couette_fixed_point():
+    cfg = small_cfg(COUETTE)
+    o, _ = make(cfg, zero_pert=True)
+    o.step(20)
+    assert np.abs(o.U - o.y).max() < 1e-13
+    assert np.abs(o.v).max() == 0.0 and np.abs(o.eta).max() == 0.0 and np.abs(o.W).max() < 1e-15
+    assert np.allclose(o.gamma, 0.0)
+
+
+@pytest.mark.parametrize("c", [1.5, 0.7])
+def test_P2_laminar_poiseuille_fixed_point_gamma(c):
+    cfg = small_cfg(POISEUILLE_CMF, Re=2800.0, dt=0.005, cid=3)
+    o = Oracle(*inputs.plan_args(cfg))
+    z = np.zeros((cfg.E, cfg.Nx // 2, cfg.Nz - 1, cfg.Ny), complex)
+    U = np.tile(c * (1 - o.y ** 2), (cfg.E, 1))
+    o.set_state(z, z, U, np.zeros_like(U))
+    o.step(20)
+    assert np.abs(o.U - U).max() < 1e-13
+    assert np.abs(o.gamma - 2 * c / cfg.Re).max() < 1e-13 * cfg.Re      # gamma = 2c/Re (reading A6)
+    d = o.diagnostics()
+    assert np.abs(d[:, 3] - 2 * c / 3).max() < 1e-13                     # bulk flux of c(1-y^2)
+    assert np.abs(d[:, 1] - 2 * c).max() < 1e-10 and np.abs(d[:, 2] + 2 * c).max() < 1e-10
+
+
+# ------------------------------------------------------------------------------------------------ P3
+def test_P3_manufactured_helmholtz_solve():
+    Ny, a = 33, 7.3
+    y = cheb_points(Ny)
+    D2 = (cheb_D(Ny) @ cheb_D(Ny))[1:-1, 1:-1]
+    v = (1 - y ** 2) * np.cos(PI * y)
+    d2v = -2 * np.cos(PI * y) + 4 * PI * y * np.sin(PI * y) - PI ** 2 * (1 - y ** 2) * np.cos(PI * y)
+    rhs = (d2v - a * v)[1:-1]
+    sol = sla.solve(D2 - a * np.eye(Ny - 2), rhs)
+    assert np.abs(sol - v[1:-1]).max() < 1e-9
+
+
+@pytest.mark.parametrize("Ny", [13, 17, 33, 49])
+def test_P3_clamped_D4_exact_on_clamped_polynomials(Ny):
+    y = cheb_points(Ny)
+    D4c = clamped_D4(Ny)
+    rng = np.random.default_rng(3)
+    env = np.array([1.0, 0, -2.0, 0, 1.0])                              # (1-y^2)^2
+    for deg in (0, 1, 3, Ny - 5):                                       # p = (1-y^2)^2 r, deg p <= Ny-1
+        r = rng.standard_normal(deg + 1)
+        p = npoly.polymul(env, r)
+        exact = npoly.polyval(y, npoly.polyder(p, 4))[1:-1]
+        got = D4c @ npoly.polyval(y, p)[1:-1]
+        scale = np.abs(D4c).max() * np.abs(npoly.polyval(y, p)).max()
+        # entries of D4c grow like Ny^8: the attainable accuracy is a few ulp of |D4c| |p|
+        assert np.abs(got - exact).max() < 2e-14 * scale, deg
+        if Ny <= 17:                                                    # tight enough to catch a wrong coefficient
+            assert np.abs(got - exact).max() < 1e-9 * np.abs(exact).max(), deg
+
+
+def test_P3_biharmonic_operator_matches_pde():
+    """Delta Delta = D4c - 2 alpha D2 + alpha^2 (reading A7) applied to a clamped, non-polynomial
+    function equals the analytic d4v - 2 alpha d2v + alpha^2 v, and T = Delta^-1 Delta Delta solves
+    Delta (T v) = Delta Delta v with (T v)(+-1) = 0."""
+    from math import comb
+    cfg = small_cfg(Ny=33)
+    o = Oracle(*inputs.plan_args(cfg))
+    y, c = o.y, 0.5
+    a = o.alpha[1, 2]
+    p = np.array([1.0, 0, -2.0, 0, 1.0])
+
+    def der(k):   # (p e^{cy})^(k) = e^{cy} sum_i C(k,i) c^(k-i) p^(i)
+        return np.exp(c * y) * sum(comb(k, i) * c ** (k - i) * npoly.polyval(y, npoly.polyder(p, i) if i else p)
+                                   for i in range(k + 1))
+
+    v = der(0)
+    bih = (der(4) - 2 * a * der(2) + a * a * v)[1:-1]
+    I = np.eye(o.Ni)
+    DelDel = o.D4c - 2 * a * o.D2 + a * a * I
+    scale = np.abs(o.D4c).max() * np.abs(v).max()
+    assert np.abs(DelDel @ v[1:-1] - bih).max() < 2e-14 * scale
+    assert np.abs(DelDel @ v[1:-1] - bih).max() < 1e-5 * np.abs(bih).max()
+    Del, T, _ = o.ops[a]
+    assert np.abs(Del @ (T @ v[1:-1]) - bih).max() < 1e-5 * np.abs(bih).max()
+
+
+# ------------------------------------------------------------------------------------------------ P4 / P5
+def _identities(o):
+    u, v, w, Du, Dv, Dw = o.velocities(o.v, o.eta, o.U, o.W)
+    ikx = 1j * o.kx[None, :, None, None]
+    ikz = 1j * o.kz[None, None, :, None]
+    div = (ikx * u + Dv + ikz * w)[..., 1:-1]
+    vort = (ikz * u - ikx * w - o.eta)[..., 1:-1]
+    div[:, 0, 0] = 0
+    vort[:, 0, 0] = 0
+    scale = max(np.abs(Dv).max(), np.abs(o.eta).max())
+    return np.abs(div).max() / scale, np.abs(vort).max() / scale, u, v, w
+
+
+@pytest.mark.parametrize("flow", [COUETTE, POISEUILLE_CMF])
+def test_P4_P5_divergence_vorticity_noslip_flux(flow):
+    cfg = small_cfg(flow, Re=600.0, dt=0.01, cid=3 if flow else 1)
+    o, st = make(cfg)
+    Q0 = 0.5 * o.U @ o.w
+    o.step(3)
+    ediv, evort, u, v, w = _identities(o)
+    assert ediv < 1e-13 and evort < 1e-13
+    # no-slip exactly, by construction (reading A10)
+    for f in (v, o.eta):
+        assert np.all(f[..., 0] == 0) and np.all(f[..., -1] == 0)
+    nz = np.ones((cfg.Nx // 2, cfg.Nz - 1), bool)
+    nz[0, 0] = False
+    assert np.all(u[:, nz][..., 0] == 0) and np.all(w[:, nz][..., -1] == 0)
+    assert np.all(o.U[:, 0] == -o.Uw) and np.all(o.U[:, -1] == o.Uw)
+    assert np.all(o.W[:, 0] == 0) and np.all(o.W[:, -1] == 0)
+    assert np.abs(o.v[:, 0, 0]).max() == 0 and np.abs(o.eta[:, 0, 0]).max() == 0
+    # physical-space divergence on the padded grid
+    ikx = 1j * o.kx[None, :, None, None]
+    ikz = 1j * o.kz[None, None, :, None]
+    _, _, _, _, Dv, _ = o.velocities(o.v, o.eta, o.U, o.W)
+    d = o.to_physical(ikx * u) + o.to_physical(Dv) + o.to_physical(ikz * w)
+    assert np.abs(d[:, 1:-1]).max() < 1e-13
+    if flow == POISEUILLE_CMF:
+        assert np.abs(0.5 * o.U @ o.w - Q0).max() < 1e-13                            # P5
+    # the n = 0 plane stays Hermitian: entries with m < 0 are conjugates of m > 0
+    for i, m in enumerate(o.m_of):
+        if m < 0:
+            assert np.abs(o.v[:, 0, i] - np.conj(o.v[:, 0, -m])).max() < 1e-15
+
+
+# ------------------------------------------------------------------------------------------------ P6
+@pytest.mark.parametrize("p", [1, 2, 3])
+def test_P6_squire_mode_crank_nicolson_factor(p):
+    cfg = small_cfg(POISEUILLE_CMF, Ny=33, Re=50.0, dt=0.05, cid=3)
+    o = Oracle(*inputs.plan_args(cfg))
+    z = np.zeros((cfg.E, cfg.Nx // 2, cfg.Nz - 1, cfg.Ny), complex)
+    eta = z.copy()
+    n, mi = 2, 1
+    prof = np.sin(p * PI * (o.y + 1) / 2)
+    eta[:, n, mi] = 1e-9 * (1 + 0.5j) * prof
+    o.set_state(z, eta, np.zeros((cfg.E, cfg.Ny)), np.zeros((cfg.E, cfg.Ny)))
+    o.step(1)
+    lam = o.alpha[n, mi] + (p * PI / 2) ** 2
+    g1 = cfg.dt / (2 * cfg.Re)
+    fac = (1 - g1 * lam) / (1 + g1 * lam)
+    err = np.abs(o.eta[:, n, mi] - fac * eta[:, n, mi]).max() / np.abs(eta[:, n, mi]).max()
+    assert err < 1e-10
+    assert np.abs(o.v).max() < 1e-20
+
+
+# ------------------------------------------------------------------------------------------------ P7
+def _cheb_vandermonde_ops(N):
+    """Independent collocation operators: differentiate the Chebyshev series (numpy.polynomial.chebyshev),
+    not the closed-form entries the oracle uses."""
+    y = -np.cos(PI * np.arange(N) / (N - 1))
+    V = C.chebvander(y, N - 1)
+    Vinv = np.linalg.inv(V)
+    eye = np.eye(N)
+    ders = []
+    for k in range(5):
+        dV = np.stack([C.chebval(y, C.chebder(eye[j], k)) if k else V[:, j] for j in range(N)], axis=1)
+        ders.append(dV @ Vinv)
+    return y, ders
+
+
+def _os_squire_eig(N, Re, kx, kz, Ufun, dUfun, d2Ufun):
+    """Generalised eigenproblem -i omega B q = L q for q = (v, eta), clamped rows replaced (independent of the
+    oracle's cheb4bc-style matrix).  Linearisation of PAPER.md Eq. 4-5 about U(y):
+      d/dt Lap v = [-i kx U Lap + i kx U'' + Lap Lap / Re] v ;  d/dt eta = [-i kx U + Lap/Re] eta - i kz U' v."""
+    y, (I, D1, D2, D3, D4) = _cheb_vandermonde_ops(N)
+    a2 = kx * kx + kz * kz
+    U, dU, d2U = np.diag(Ufun(y)), np.diag(dUfun(y)), np.diag(d2Ufun(y))
+    Lap = D2 - a2 * I
+    LapLap = D4 - 2 * a2 * D2 + a2 * a2 * I
+    Los = -1j * kx * U @ Lap + 1j * kx * d2U + LapLap / Re
+    Lsq = -1j * kx * U + Lap / Re
+    Z = np.zeros((N, N))
+    A = np.block([[Los, Z], [-1j * kz * dU, Lsq]]).astype(complex)
+    B = np.block([[Lap, Z], [Z, I]]).astype(complex)
+    big = -1e4                                  # spurious boundary eigenvalues pushed far into the stable half
+    for r, row in ((0, I[0]), (N - 1, I[-1]), (1, D1[0]), (N - 2, D1[-1])):
+        A[r, :] = 0
+        B[r, :] = 0
+        A[r, :N] = big * row
+        B[r, :N] = row
+    for r in (N, 2 * N - 1):
+        A[r, :] = 0
+        B[r, :] = 0
+        A[r, N:] = big * I[r - N]
+        B[r, N:] = I[r - N]
+    lam, vec = sla.eig(A, B)                    # d/dt q = lam q
+    ok = np.isfinite(lam) & (lam.real > -50)
+    lam, vec = lam[ok], vec[:, ok]
+    return y, lam, vec
+
+
+def _read_golden(name):
+    vals = {}
+    with open(os.path.join(GOLDEN, name)) as f:
+        for line in f:
+            if line.startswith("#") or not line.strip():
+                continue
+            k, v = line.split()
+            vals[k] = float(v)
+    return vals
+
+
+def test_P7_independent_eigensolver_reproduces_orszag():
+    g = _read_golden("orszag1971_poiseuille_Re10000.txt")
+    _, lam, _ = _os_squire_eig(121, 1e4, 1.0, 0.0, lambda y: 1 - y * y, lambda y: -2 * y, lambda y: -2 + 0 * y)
+    c = 1j * lam / 1.0                          # lam = -i omega = -i kx c
+    best = c[np.argmax(c.imag)]
+    assert abs(best.real - g["c_real"]) < 2e-7 and abs(best.imag - g["c_imag"]) < 2e-7
+
+
+@pytest.mark.parametrize("flow,Re,n,m", [(POISEUILLE_CMF, 3000.0, 1, 1), (COUETTE, 800.0, 1, 2),
+                                          (POISEUILLE_CMF, 10000.0, 1, 0)])
+def test_P7_oracle_growth_rate_matches_orr_sommerfeld_squire(flow, Re, n, m):
+    Lx, Lz = 2 * PI, 2 * PI
+    Ny = 81 if Re > 5000 else 57
+    dt, nsteps = 0.01, 40
+    if flow == POISEUILLE_CMF:
+        Uf, dUf, d2Uf = (lambda y: 1 - y * y), (lambda y: -2 * y), (lambda y: -2 + 0 * y)
+    else:
+        Uf, dUf, d2Uf = (lambda y: y), (lambda y: 1 + 0 * y), (lambda y: 0 * y)
+    kx, kz = 2 * PI * n / Lx, 2 * PI * m / Lz
+    Neig = Ny + 24                               # a different resolution from the oracle's
+    yE, lam, vec = _os_squire_eig(Neig, Re, kx, kz, Uf, dUf, d2Uf)
+    # least-stable mode with a non-trivial v component (an Orr-Sommerfeld mode with its forced eta)
+    vnorm = np.linalg.norm(vec[:Neig], axis=0) / np.linalg.norm(vec, axis=0)
+    cand = np.where(vnorm > 1e-3)[0]
+    k = cand[np.argmax(lam[cand].real)]
+    lam_k = lam[k]
+    if flow == POISEUILLE_CMF and m == 0 and Re == 10000.0:
+        g = _read_golden("orszag1971_poiseuille_Re10000.txt")
+        assert abs(1j * lam_k / kx - (g["c_real"] + 1j * g["c_imag"])) < 1e-6
+    # interpolate the eigenfunction to the oracle grid through its Chebyshev series
+    Vinv = np.linalg.inv(C.chebvander(yE, Neig - 1))
+    o = Oracle(12, Ny, 12, 1, Re, Lx, Lz, dt, flow)
+    cv, ce = Vinv @ vec[:Neig, k], Vinv @ vec[Neig:, k]
+    v0 = C.chebval(o.y, cv)
+    e0 = C.chebval(o.y, ce)
+    amp = 1e-8 / np.abs(v0).max()
+    vh = np.zeros((1, 6, 11, Ny), complex)
+    eh = np.zeros_like(vh)
+    mi = inputs.m_index(m, 12)
+    vh[0, n, mi], eh[0, n, mi] = amp * v0, amp * e0
+    o.set_state(vh, eh, Uf(o.y)[None], np.zeros((1, Ny)))
+    v_init, e_init = o.v[0, n, mi].copy(), o.eta[0, n, mi].copy()
+    o.step(nsteps)
+    T = nsteps * dt
+    # project on the initial shape: complex amplification factor
+    fac_v = np.vdot(v_init, o.v[0, n, mi]) / np.vdot(v_init, v_init)
+    expect = np.exp(lam_k * T)
+    assert abs(fac_v - expect) < 2e-6 * abs(expect), (fac_v, expect)
+    if m != 0:
+        fac_e = np.vdot(e_init, o.eta[0, n, mi]) / np.vdot(e_init, e_init)
+        assert abs(fac_e - expect) < 2e-6 * abs(expect), (fac_e, expect)
+    # shape preserved (it is an eigenfunction): residual orthogonal to the initial shape is tiny
+    res = o.v[0, n, mi] - fac_v * v_init
+    assert np.linalg.norm(res) < 1e-5 * np.linalg.norm(v_init)
+    # laminar base flow untouched at O(amp^2)
+    assert np.abs(o.U[0] - Uf(o.y)).max() < 1e-12
+
+
+# ------------------------------------------------------------------------------------------------ P8
+def test_P8_temporal_order_two():
+    base = small_cfg(COUETTE, Re=300.0, rms=0.2)
+    T = 0.16
+
+    def run(dt):
+        cfg = inputs.Config(**{**base.__dict__, "dt": dt})
+        o, _ = make(cfg)
+        o.step(int(round(T / dt)))
+        return o.v.copy(), o.eta.copy(), o.U.copy()
+
+    ref = run(0.0025)
+    errs = []
+    for dt in (0.04, 0.02, 0.01):
+        r = run(dt)
+        errs.append(max(np.abs(r[0] - ref[0]).max(), np.abs(r[1] - ref[1]).max(), np.abs(r[2] - ref[2]).max()))
+    r1, r2 = errs[0] / errs[1], errs[1] / errs[2]
+    assert 3.3 < r1 < 5.0 and 3.3 < r2 < 5.2, (errs, r1, r2)
+
+
+# ------------------------------------------------------------------------------------------------ P9 / P14
+def test_P14_single_harmonic_dft_roundtrip():
+    cfg = small_cfg()
+    o = Oracle(*inputs.plan_args(cfg))
+    fh = np.zeros((1, o.nkx, o.nkz, o.Ny), complex)
+    n, mi = 3, inputs.m_index(-2, cfg.Nz)
+    fh[0, n, mi, :] = 0.3 - 0.7j
+    f = o.to_physical(fh)
+    x = 2 * PI * np.arange(o.Mx) / o.Mx
+    z = 2 * PI * np.arange(o.Mz) / o.Mz
+    exact = 2 * np.real((0.3 - 0.7j) * np.exp(1j * (3 * x[:, None] - 2 * z[None, :])))
+    assert np.abs(f[0, 5] - exact).max() < 1e-14
+    back = o.to_spectral(f)
+    assert np.abs(back - fh).max() < 1e-14
+    assert np.abs(dft_matrix(np.array([1]), 8, +1)[0, 2] - 1j) < 1e-15          # sign of the exponent (A5)
+
+
+def test_P9_dealiasing_cutoff():
+    cfg = small_cfg(Nx=16, Nz=16)
+    o = Oracle(*inputs.plan_args(cfg))
+    a, b = 0.4 + 0.2j, -0.3 + 0.9j
+    for (n1, n2) in ((7, 5), (7, 7), (4, 6)):
+        f1 = np.zeros((1, o.nkx, o.nkz, o.Ny), complex)
+        f2 = np.zeros_like(f1)
+        f1[0, n1, 0, :] = a
+        f2[0, n2, 0, :] = b
+        prod = o.to_spectral(o.to_physical(f1) * o.to_physical(f2))
+        expect = np.zeros_like(prod)
+        if n1 + n2 <= o.nkx - 1:
+            expect[0, n1 + n2, 0, :] += a * b
+        d = abs(n1 - n2)
+        expect[0, d, 0, :] += (a * np.conj(b) if n1 >= n2 else np.conj(a) * b) if d else 2 * np.real(a * np.conj(b))
+        assert np.abs(prod - expect).max() < 1e-14, (n1, n2)
+    # same in z with negative modes
+    f1 = np.zeros((1, o.nkx, o.nkz, o.Ny), complex)
+    f2 = np.zeros_like(f1)
+    f1[0, 1, inputs.m_index(7, 16), :] = a
+    f2[0, 2, inputs.m_index(6, 16), :] = b
+    prod = o.to_spectral(o.to_physical(f1) * o.to_physical(f2))
+    expect = np.zeros_like(prod)
+    expect[0, 1, inputs.m_index(-1, 16), :] = np.conj(a) * b          # (2,6)-(1,7) = (1,-1); sum (3,13) is cut
+    assert np.abs(prod - expect).max() < 1e-14
+
+
+# ------------------------------------------------------------------------------------------------ P10
+def test_P10_translation_and_reflection_covariance():
+    cfg = small_cfg(COUETTE, Re=500.0, rms=0.1)
+    o, st = make(cfg)
+    o.step(2)
+    # x-translation by s:  fhat -> fhat exp(-i kx s)
+    s = 0.37
+    ph = np.exp(-1j * o.kx * s)[None, :, None, None]
+    o2 = Oracle(*inputs.plan_args(cfg))
+    o2.set_state(st["vhat"] * ph, st["etahat"] * ph, st["U00"], st["W00"])
+    o2.step(2)
+    assert np.abs(o2.v - o.v * ph).max() < 1e-12 and np.abs(o2.eta - o.eta * ph).max() < 1e-12
+    assert np.abs(o2.U - o.U).max() < 1e-13
+    # reflection z -> -z:  v(n,m) -> v(n,-m), eta -> -eta(n,-m), W -> -W
+    mneg = np.array([inputs.m_index(-m, cfg.Nz) for m in o.m_of])
+    o3 = Oracle(*inputs.plan_args(cfg))
+    o3.set_state(st["vhat"][:, :, mneg], -st["etahat"][:, :, mneg], st["U00"], -st["W00"])
+    o3.step(2)
+    assert np.abs(o3.v - o.v[:, :, mneg]).max() < 1e-12
+    assert np.abs(o3.eta + o.eta[:, :, mneg]).max() < 1e-12
+    assert np.abs(o3.W + o.W).max() < 1e-13
+
+
+# ------------------------------------------------------------------------------------------------ P11
+def _budget_rhs(o):
+    """-eps + wall work + gamma U_b with eps = (Re V)^-1 int |grad u|^2, evaluated spectrally."""
+    u, v, w, Du, Dv, Dw = o.velocities(o.v, o.eta, o.U, o.W)
+    al = o.alpha[None, :, :, None]
+    cn = np.where(o.n_of == 0, 1.0, 2.0)[None, :, None, None]
+    g2 = al * (abs(u) ** 2 + abs(v) ** 2 + abs(w) ** 2) + abs(Du) ** 2 + abs(Dv) ** 2 + abs(Dw) ** 2
+    eps = 0.5 * np.einsum("enmj,j->e", cn * g2, o.w) / o.Re
+    dU = o.U @ o.D.T
+    wall = o.Uw / (2 * o.Re) * (dU[:, -1] + dU[:, 0])
+    Ub = 0.5 * o.U @ o.w
+    return -eps + wall + o.gamma * Ub
+
+
+def test_P11_laminar_budget_closed_forms():
+    for flow, c, expect in ((COUETTE, None, 1.0), (POISEUILLE_CMF, 1.0, 4.0 / 3.0)):
+        cfg = small_cfg(flow, Re=100.0, cid=3 if flow else 1)
+        o = Oracle(*inputs.plan_args(cfg))
+        z = np.zeros((cfg.E, cfg.Nx // 2, cfg.Nz - 1, cfg.Ny), complex)
+        U = np.tile(o.y if flow == COUETTE else (1 - o.y ** 2), (cfg.E, 1))
+        o.set_state(z, z, U, 0 * U)
+        o.step(1)
+        u, v, w, Du, Dv, Dw = o.velocities(o.v, o.eta, o.U, o.W)
+        eps = 0.5 * np.einsum("ej,j->e", abs(Du[:, 0, 0]) ** 2, o.w) / o.Re
+        assert np.abs(eps - expect / cfg.Re).max() < 1e-13                  # dissipation 1/Re and 4/(3Re)
+        assert np.abs(_budget_rhs(o)).max() < 1e-13                         # input balances dissipation
+
+
+@pytest.mark.parametrize("flow", [COUETTE, POISEUILLE_CMF])
+def test_P11_energy_budget_across_a_step(flow):
+    res = []
+    for dt in (0.02, 0.01):
+        cfg = small_cfg(flow, Re=200.0, dt=dt, rms=0.3, cid=3 if flow else 1)
+        o, _ = make(cfg)
+        o.step(2)                                                           # so that gamma is defined
+        E0, r0 = o.energy(), _budget_rhs(o)
+        o.step(1)
+        E1, r1 = o.energy(), _budget_rhs(o)
+        res.append(np.abs((E1 - E0) - 0.5 * dt * (r0 + r1)).max())
+        assert res[-1] < 5e-3 * np.abs(dt * r0).max() + 1e-9
+    assert res[0] / res[1] > 5.0, res                                       # trapezoid residual ~ dt^3
+
+
+# ------------------------------------------------------------------------------------------------ P12 / P13
+def test_P12_member_independence():
+    cfg = small_cfg(E=3)
+    o, _ = make(cfg)
+    o.step(2)
+    o1, _ = make(cfg, members=[1])
+    o1.step(2)
+    assert np.array_equal(o1.v[0], o.v[1]) or np.abs(o1.v[0] - o.v[1]).max() < 1e-15
+    assert np.abs(o1.eta[0] - o.eta[1]).max() < 1e-15 and np.abs(o1.U[0] - o.U[1]).max() < 1e-15
+
+
+def test_P13_lu_path_vs_explicit_inverses():
+    """Brute force on a tiny case: the stage written with explicitly inverted matrices (the form the paper
+    and the GPU path multiply with, Listing 3) equals the oracle's LU path."""
+    cfg = small_cfg(POISEUILLE_CMF, Nx=12, Ny=13, Nz=12, Re=300.0, cid=3)
+    o, _ = make(cfg)
+    F, G, Su, Sw = o.nonlinear(o.v, o.eta, o.U, o.W)
+    h = 0.5
+    v1, e1, U1, W1, gam = o.stage(o.v, o.eta, o.U, o.W, h, F, G, Su, Sw)
+    I = np.eye(o.Ni)
+    g = h * o.dt / (2 * o.Re)
+    for n, mi in ((1, 2), (3, 9), (0, 4)):
+        a = o.alpha[n, mi]
+        Del = o.D2 - a * I
+        T = np.linalg.inv(Del) @ (o.D4c - 2 * a * o.D2 + a * a * I)
+        Ainv = np.linalg.inv(I - g * T)
+        vv = (Ainv @ (I + g * T)) @ o.v[:, n, mi, 1:-1].T + (-h * o.dt * Ainv @ np.linalg.inv(Del)) @ F[:, n, mi].T
+        ICg = np.linalg.inv(I - g * Del)
+        ee = (ICg @ (I + g * Del)) @ o.eta[:, n, mi, 1:-1].T + (-h * o.dt * ICg) @ G[:, n, mi].T
+        assert np.abs(vv.T - v1[:, n, mi, 1:-1]).max() < 1e-12 * max(1, np.abs(v1).max())
+        assert np.abs(ee.T - e1[:, n, mi, 1:-1]).max() < 1e-12 * max(1, np.abs(e1).max())
+
+
+def test_generator_energy_closed_form_matches_oracle_energy():
+    """The generator scales each member with exact polynomial integrals; the oracle's spectral energy of the
+    perturbation (total minus laminar, no cross term) must reproduce the requested rms."""
+    for cid in (1, 3):
+        base = inputs.CONFIGS[cid]
+        cfg = inputs.Config(**{**base.__dict__, "Nx": 16, "Nz": 16, "Ny": 33, "E": 2})
+        o, st = make(cfg)
+        lam = Oracle(*inputs.plan_args(cfg))
+        z = np.zeros_like(st["vhat"])
+        lam.set_state(z, z, st["U00"], st["W00"])
+        rms = np.sqrt(2 * (o.energy() - lam.energy()))
+        assert np.abs(rms - st["rms"]).max() < 1e-9
