@@ -1,0 +1,133 @@
+/* dns.h -- C ABI of libdns_b200: the vectorised ensemble time step of arXiv 2306.12739
+ * ("A vectorized Navier-Stokes ensemble DNS code for plane parallel flows") on one NVIDIA B200 (sm_100a).
+ *
+ * The library advances E independent realisations of 3-D incompressible plane Couette / constant-mass-flux
+ * Poiseuille flow at once.  State = wall-normal velocity v and wall-normal vorticity eta (PAPER.md:68,
+ * Eq. 4-5 :72-74) in Fourier space in x,z and on Ny Chebyshev-Gauss-Lobatto points in y, plus the mean
+ * profiles U00(y), W00(y) (Eq. 6-7 :76-78).  Time stepping is the combined Crank-Nicolson / 3rd-order
+ * Runge-Kutta scheme (Eq. 11); next-stage fields come from precomputed per-(kx,kz) matrix
+ * inverses (Eq. 12-15 :153-163, Listings 3-5) applied to all members at once.
+ *
+ * Every entry point returns an int status (DNS_OK = 0, negative on error); nothing throws or aborts across
+ * the ABI.  No torch / C++ types appear in the signatures.  All compute runs in the library's CUDA kernels;
+ * there is no CPU fallback: without a CUDA device every call that needs one returns DNS_ECUDA.
+ *
+ * Array layouts at the ABI (C order, last index fastest):
+ *   vhat, etahat : [E][nkx][nkz][Ny] complex128 as interleaved (re, im) doubles
+ *                  nkx = Nx/2, streamwise mode n = 0 .. Nx/2-1            (kx = 2 pi n / Lx)
+ *                  nkz = Nz-1, spanwise mode m in FFT order 0,1,..,Nz/2-1, -(Nz/2-1),..,-1
+ *                                                                       (kz = 2 pi m / Lz; `mrange`)
+ *                  y_j = -cos(pi j/(Ny-1)), j = 0..Ny-1, ascending from the lower wall
+ *   U00, W00     : [E][Ny] float64
+ * Fourier convention: f(x,z) = sum_{n,m} fhat(n,m) exp(+i(kx x + kz z)); coefficients are amplitudes; only
+ * n >= 0 is stored, fhat(-n,-m) = conj fhat(n,m).  The Nyquist modes n = Nx/2, m = -Nz/2 are not stored and
+ * are identically zero (3/2-rule dealiasing on an Mx = 3Nx/2, Mz = 3Nz/2 grid).
+ * Pointers passed to set/get/diagnostics may be HOST or DEVICE pointers (detected with
+ * cudaPointerGetAttributes); the caller owns them and the library keeps no reference after the call returns.
+ */
+#ifndef DNS_B200_H
+#define DNS_B200_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct dns_plan dns_plan; /* opaque, owned by the library */
+
+enum { DNS_COUETTE = 0, DNS_POISEUILLE_CMF = 1 }; /* flow */
+
+enum {
+    DNS_OK = 0,
+    DNS_EINVAL = -1,     /* bad argument (see each call) */
+    DNS_ENOMEM = -2,     /* host or device allocation failed */
+    DNS_ECUDA = -3,      /* CUDA runtime error or no device; sticky on the plan */
+    DNS_ENONFINITE = -4, /* a member's energy is not finite (dns_diagnostics) */
+    DNS_ESTATE = -5      /* call out of order (no workspace bound, no state set) */
+};
+
+/* kernel classes reported by dns_step_profile (north_star subsystems (1)-(4)) */
+enum {
+    DNS_CLASS_FFT_Z_INV = 0, /* a4, z direction: zero-pad + i kz + complex inverse FFT            */
+    DNS_CLASS_LINE = 1,      /* a4 x direction + a5 products + a6 x direction, fused per (y,z) line */
+    DNS_CLASS_FFT_Z_FWD = 2, /* a6, z direction: forward FFT + truncation + 1/(Mx Mz)              */
+    DNS_CLASS_YPAIR = 3,     /* a7,a8,a9,a1,a2,a3: per-(kx,kz) DMMA contractions + stage algebra   */
+    DNS_CLASS_MEAN = 4,      /* a10: mean flow, wall lift, mass-flux gamma                          */
+    DNS_NCLASS = 5
+};
+
+/* dns_plan_create -- precompute everything that is constant for a fixed dt: Chebyshev D,
+ * D2 = D*D, the clamped fourth derivative, and for every distinct
+ * alpha = kx^2+kz^2 and h in {1/2, 1} the inverses of Eq. 12-13 (Listing 3) and of the
+ * mean-flow operator of Eq. 14-15; uploads them to the current CUDA device.
+ *   Nx, Nz : un-padded Fourier grid, even; Mx = 3Nx/2 and Mz = 3Nz/2 must be 2^a 3^b within 16..128
+ *   Ny     : Chebyshev-Gauss-Lobatto points including both walls, 5 <= Ny <= 257
+ *   E      : ensemble members (PAPER.md:131 `Fn`), >= 1
+ *   Re     : 1/nu in the units of the state; Lx, Lz periodic lengths (y in [-1,1]); dt fixed step
+ *   flow   : DNS_COUETTE (walls at +-1 move with U = +-1, gamma = 0) or DNS_POISEUILLE_CMF (walls at rest,
+ *            gamma(t) solved every stage so that the bulk flux (1/2) int U00 dy keeps the value it had in
+ *            dns_set_state)
+ * Errors: DNS_EINVAL (null out, bad sizes, non-positive Re/Lx/Lz/dt, unknown flow), DNS_ENOMEM, DNS_ECUDA.
+ * On success *out owns host and device memory until dns_plan_destroy. */
+int dns_plan_create(dns_plan** out, int Nx, int Ny, int Nz, int E, double Re, double Lx, double Lz, double dt,
+                    int flow);
+
+/* Bytes of DEVICE workspace the caller must provide to dns_plan_bind (state, stage buffers, transform
+ * intermediates).  0 if plan is null. */
+size_t dns_plan_workspace_bytes(const dns_plan* plan);
+
+/* dns_plan_bind -- hand the plan a device buffer (256-byte aligned, >= dns_plan_workspace_bytes) and the CUDA
+ * stream (cudaStream_t as void*, NULL = default stream) every later call works on.  The buffer stays owned by
+ * the caller and must outlive the plan or the next bind; it is zero-filled here.
+ * Errors: DNS_EINVAL (null plan/buffer, too small, misaligned), DNS_ECUDA. */
+int dns_plan_bind(dns_plan* plan, void* dev_workspace, size_t bytes, void* cuda_stream);
+
+/* dns_set_state -- load the state at time t = 0 (ABI layout above; host or device pointers).  Input is
+ * normalised: wall rows of vhat, etahat and their (0,0) column are set to 0 (PAPER.md:82 Eq. 8, :87); wall rows
+ * of U00 to -+1 (Couette) or 0, of W00 to 0 (Eq. 9 :85); on the n = 0 plane entries with m < 0 are replaced by
+ * the conjugates of m > 0.  The Poiseuille target flux of member e is the Clenshaw-Curtis bulk mean of U00[e].
+ * Also derives u, w, dU/dy ... needed by the first nonlinear evaluation (Eq. 17-18 :214-216).  Asynchronous
+ * for device pointers; for host pointers the copies are enqueued on the plan's stream and synchronised.
+ * Errors: DNS_EINVAL (null), DNS_ESTATE (no workspace), DNS_ECUDA. */
+int dns_set_state(dns_plan* plan, const double* vhat, const double* etahat, const double* U00,
+                  const double* W00);
+
+/* dns_step -- enqueue nsteps full CN/RK3 time steps (3 stages each) on the plan's stream
+ * and return without synchronising.  Errors: DNS_EINVAL (nsteps < 0), DNS_ESTATE (no state), DNS_ECUDA. */
+int dns_step(dns_plan* plan, int nsteps);
+
+/* dns_step_profile -- as dns_step, but brackets every kernel class with CUDA events on the plan's stream,
+ * synchronises, and adds the elapsed milliseconds per class to ms_by_class[DNS_NCLASS] (host array). */
+int dns_step_profile(dns_plan* plan, int nsteps, double* ms_by_class);
+
+/* dns_get_state -- copy the current state out (same layout as dns_set_state; any pointer may be NULL to skip
+ * that array); synchronises the stream.  Errors: DNS_ESTATE, DNS_ECUDA. */
+int dns_get_state(dns_plan* plan, double* vhat, double* etahat, double* U00, double* W00);
+
+/* dns_diagnostics -- out[E][6] (host or device): [0] kinetic energy 1/(2V) int |u|^2 dV,
+ * [1] dU00/dy at the lower wall, [2] at the upper wall (tau_w = (1/Re) dU00/dy), [3] bulk flux
+ * (1/2) int U00 dy, [4] gamma used in the last stage, [5] time t.  Synchronises.
+ * Returns DNS_ENONFINITE if any member's energy is not finite (rows are still filled). */
+int dns_diagnostics(dns_plan* plan, double* out);
+
+/* dns_debug_fetch -- test hook: copy one INTERNAL device array to a host buffer, synchronising first.  Internal
+ * spectral layout is [Ny][nkx][nkz][E] complex128 (member index fastest).  which: 0 u, 1 w, 2 du/dy, 3 dw/dy
+ * (current stage, Eq. 17-18), 4 the three spectral advection terms (u.grad)u,(u.grad)v,(u.grad)w back to back,
+ * 5 F^0, 6 G^0 (stage-0 nonlinear terms of Eq. 4-5, interior rows), 7 v of the current stage, 8 U00 and
+ * 9 W00 of the current stage as [Ny][E] float64.  nbytes must equal the array size (DNS_EINVAL otherwise). */
+int dns_debug_fetch(dns_plan* plan, int which, void* host_dst, size_t nbytes);
+
+/* Number of kernel launches one dns_step(1) enqueues (for bench.py's gpu_launches). */
+int dns_launches_per_step(const dns_plan* plan);
+
+/* Frees plan-owned host and device memory (not the bound workspace).  Null is accepted. */
+int dns_plan_destroy(dns_plan* plan);
+
+/* Static string for a status code. */
+const char* dns_strerror(int status);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DNS_B200_H */

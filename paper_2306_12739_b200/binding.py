@@ -1,0 +1,220 @@
+"""Thin ctypes binding of libdns_b200.so (include/dns.h): argument marshalling only -- every step of the path
+runs in the library's CUDA kernels.  There is NO CPU fallback: if the shared library is missing the import of
+any entry point raises, and without a CUDA device dns_plan_create returns DNS_ECUDA (raised as DnsError).
+
+Module-level functions carry the C names (dns_plan_create, dns_plan_bind, dns_set_state, dns_step,
+dns_get_state, dns_diagnostics, ...); `Plan` is a small convenience wrapper that allocates the device
+workspace with torch (PyTorch is used for device memory and streams only).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+DNS_COUETTE, DNS_POISEUILLE_CMF = 0, 1
+DNS_OK, DNS_EINVAL, DNS_ENOMEM, DNS_ECUDA, DNS_ENONFINITE, DNS_ESTATE = 0, -1, -2, -3, -4, -5
+DNS_NCLASS = 5
+CLASS_NAMES = ("fft_z_inv", "line_fft_x_products", "fft_z_fwd", "ypair_dmma", "mean_flow")
+
+_LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libdns_b200.so")
+_lib = None
+
+EXPORTS = ("dns_plan_create", "dns_plan_workspace_bytes", "dns_plan_bind", "dns_set_state", "dns_step",
+           "dns_step_profile", "dns_get_state", "dns_diagnostics", "dns_debug_fetch", "dns_launches_per_step", "dns_plan_destroy",
+           "dns_strerror")
+
+
+class DnsError(RuntimeError):
+    def __init__(self, status, where):
+        self.status = status
+        super().__init__(f"{where}: {dns_strerror(status)} ({status})")
+
+
+def lib():
+    """Loads libdns_b200.so; fails loudly when it has not been built (python -m paper_2306_12739_b200.build)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_LIB_PATH):
+            raise RuntimeError(f"{_LIB_PATH} is missing: build it with `python -m paper_2306_12739_b200.build` "
+                               "(there is no CPU fallback)")
+        L = ctypes.CDLL(_LIB_PATH)
+        vp, dp, i, d = ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int, ctypes.c_double
+        L.dns_plan_create.argtypes = [ctypes.POINTER(vp), i, i, i, i, d, d, d, d, i]
+        L.dns_plan_create.restype = i
+        L.dns_plan_workspace_bytes.argtypes = [vp]
+        L.dns_plan_workspace_bytes.restype = ctypes.c_size_t
+        L.dns_plan_bind.argtypes = [vp, vp, ctypes.c_size_t, vp]
+        L.dns_plan_bind.restype = i
+        L.dns_set_state.argtypes = [vp, dp, dp, dp, dp]
+        L.dns_set_state.restype = i
+        L.dns_step.argtypes = [vp, i]
+        L.dns_step.restype = i
+        L.dns_step_profile.argtypes = [vp, i, dp]
+        L.dns_step_profile.restype = i
+        L.dns_get_state.argtypes = [vp, dp, dp, dp, dp]
+        L.dns_get_state.restype = i
+        L.dns_diagnostics.argtypes = [vp, dp]
+        L.dns_diagnostics.restype = i
+        L.dns_debug_fetch.argtypes = [vp, i, vp, ctypes.c_size_t]
+        L.dns_debug_fetch.restype = i
+        L.dns_launches_per_step.argtypes = [vp]
+        L.dns_launches_per_step.restype = i
+        L.dns_plan_destroy.argtypes = [vp]
+        L.dns_plan_destroy.restype = i
+        L.dns_strerror.argtypes = [i]
+        L.dns_strerror.restype = ctypes.c_char_p
+        _lib = L
+    return _lib
+
+
+def _ptr(a):
+    """Address of a numpy array (host) or torch tensor (host or device); None -> NULL."""
+    if a is None:
+        return None
+    if isinstance(a, np.ndarray):
+        assert a.flags["C_CONTIGUOUS"]
+        return ctypes.c_void_p(a.ctypes.data)
+    return ctypes.c_void_p(a.data_ptr())          # torch tensor
+
+
+def dns_strerror(status: int) -> str:
+    return lib().dns_strerror(int(status)).decode()
+
+
+def dns_plan_create(Nx, Ny, Nz, E, Re, Lx, Lz, dt, flow):
+    h = ctypes.c_void_p()
+    st = lib().dns_plan_create(ctypes.byref(h), int(Nx), int(Ny), int(Nz), int(E), float(Re), float(Lx), float(Lz),
+                               float(dt), int(flow))
+    return st, h
+
+
+def dns_plan_workspace_bytes(h) -> int:
+    return int(lib().dns_plan_workspace_bytes(h))
+
+
+def dns_plan_bind(h, dev_ptr: int, nbytes: int, stream: int = 0) -> int:
+    return lib().dns_plan_bind(h, ctypes.c_void_p(dev_ptr), ctypes.c_size_t(nbytes), ctypes.c_void_p(stream))
+
+
+def dns_set_state(h, vhat, etahat, U00, W00) -> int:
+    return lib().dns_set_state(h, _ptr(vhat), _ptr(etahat), _ptr(U00), _ptr(W00))
+
+
+def dns_step(h, nsteps: int) -> int:
+    return lib().dns_step(h, int(nsteps))
+
+
+def dns_step_profile(h, nsteps: int, ms: np.ndarray) -> int:
+    return lib().dns_step_profile(h, int(nsteps), _ptr(ms))
+
+
+def dns_get_state(h, vhat, etahat, U00, W00) -> int:
+    return lib().dns_get_state(h, _ptr(vhat), _ptr(etahat), _ptr(U00), _ptr(W00))
+
+
+def dns_diagnostics(h, out) -> int:
+    return lib().dns_diagnostics(h, _ptr(out))
+
+
+def dns_debug_fetch(h, which: int, out: np.ndarray) -> int:
+    return lib().dns_debug_fetch(h, int(which), _ptr(out), ctypes.c_size_t(out.nbytes))
+
+
+def dns_launches_per_step(h) -> int:
+    return lib().dns_launches_per_step(h)
+
+
+def dns_plan_destroy(h) -> int:
+    return lib().dns_plan_destroy(h)
+
+
+class Plan:
+    """dns_plan_create + a torch-allocated workspace bound on torch's current stream."""
+
+    def __init__(self, Nx, Ny, Nz, E, Re, Lx, Lz, dt, flow, device="cuda:0"):
+        import torch
+
+        self.shape = (int(E), int(Nx) // 2, int(Nz) - 1, int(Ny))
+        self.E, self.Ny = int(E), int(Ny)
+        self.device = torch.device(device)
+        self.h = None
+        if not torch.cuda.is_available():
+            raise DnsError(DNS_ECUDA, "Plan (no CUDA device; this library has no CPU path)")
+        torch.cuda.set_device(self.device)
+        st, h = dns_plan_create(Nx, Ny, Nz, E, Re, Lx, Lz, dt, flow)
+        if st != DNS_OK:
+            raise DnsError(st, "dns_plan_create")
+        self.h = h
+        nbytes = dns_plan_workspace_bytes(h)
+        self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        base = (self.workspace.data_ptr() + 255) & ~255
+        self.stream = torch.cuda.current_stream(self.device)
+        st = dns_plan_bind(h, base, nbytes, self.stream.cuda_stream)
+        if st != DNS_OK:
+            raise DnsError(st, "dns_plan_bind")
+        self.workspace_bytes = nbytes
+
+    def _chk(self, st, where):
+        if st != DNS_OK:
+            raise DnsError(st, where)
+
+    def set_state(self, vhat, etahat, U00, W00):
+        if isinstance(vhat, np.ndarray):
+            vhat = np.ascontiguousarray(vhat, dtype=np.complex128)
+            etahat = np.ascontiguousarray(etahat, dtype=np.complex128)
+            U00 = np.ascontiguousarray(U00, dtype=np.float64)
+            W00 = np.ascontiguousarray(W00, dtype=np.float64)
+            assert vhat.shape == self.shape and etahat.shape == self.shape
+            assert U00.shape == (self.E, self.Ny) and W00.shape == (self.E, self.Ny)
+        self._chk(dns_set_state(self.h, vhat, etahat, U00, W00), "dns_set_state")
+
+    def step(self, nsteps=1):
+        self._chk(dns_step(self.h, nsteps), "dns_step")
+
+    def step_profile(self, nsteps=1):
+        ms = np.zeros(DNS_NCLASS)
+        self._chk(dns_step_profile(self.h, nsteps, ms), "dns_step_profile")
+        return dict(zip(CLASS_NAMES, ms.tolist()))
+
+    def get_state(self, out=None):
+        if out is None:
+            out = (np.empty(self.shape, np.complex128), np.empty(self.shape, np.complex128),
+                   np.empty((self.E, self.Ny)), np.empty((self.E, self.Ny)))
+        self._chk(dns_get_state(self.h, *out), "dns_get_state")
+        return out
+
+    def diagnostics(self):
+        out = np.empty((self.E, 6))
+        st = dns_diagnostics(self.h, out)
+        if st not in (DNS_OK, DNS_ENONFINITE):
+            raise DnsError(st, "dns_diagnostics")
+        return out
+
+    def debug_fetch(self, which):
+        """Internal arrays (test hook): spectral ones come back in ABI order [E][nkx][nkz][Ny]."""
+        E, nkx, nkz, Ny = self.shape
+        if which in (8, 9):
+            out = np.empty((Ny, E))
+            self._chk(dns_debug_fetch(self.h, which, out), "dns_debug_fetch")
+            return np.ascontiguousarray(out.T)
+        nf = 3 if which == 4 else 1
+        out = np.empty((nf, Ny, nkx, nkz, E), np.complex128)
+        self._chk(dns_debug_fetch(self.h, which, out), "dns_debug_fetch")
+        out = np.ascontiguousarray(out.transpose(0, 4, 2, 3, 1))
+        return out if nf > 1 else out[0]
+
+    def launches_per_step(self):
+        return dns_launches_per_step(self.h)
+
+    def close(self):
+        if self.h is not None:
+            dns_plan_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

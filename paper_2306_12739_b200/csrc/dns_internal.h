@@ -1,0 +1,78 @@
+// Internal declarations shared by the translation units of libdns_b200 (not part of the ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <cstddef>
+#include <vector>
+
+#include "../../include/dns.h"
+
+// Everything a kernel needs, passed by value.  Spectral arrays are [Ny][nkx][nkz][E] complex (member index
+// fastest: the paper's vectorised-ensemble axis, is the coalescing axis); mixed (kx, z) arrays
+// are [Ny][Mz][nkx][E] complex; mean-flow arrays are [Ny][E] real.
+struct DnsDev {
+    int Nx, Ny, Nz, E, Mx, Mz, nkx, nkz, nzh, P, Ni, flow;
+    double dt, Re, Uw, invMxMz;
+    // plan-owned constant tables
+    const double* kx;      // [nkx]
+    const double* kz;      // [nkz] (FFT order)
+    const double* w;       // [Ny] Clenshaw-Curtis weights
+    const double* Dfull;   // [Ny][Ny]
+    const double* Dii;     // [Ni][Ni] interior block of D
+    const double* mats;    // [2 (h=1/2,1)][nkx*nzh][3 (Ainv, Ainv*Delinv, Sinv)][Ni*Ni]
+    const double* S0inv;   // [2][Ni*Ni]
+    const double* bc;      // [2][Ni]   S0m[int,0]*U_lo + S0m[int,Ny-1]*U_hi
+    const double* Ugam;    // [2][Ni]   S0inv * (h dt 1)
+    double wUg[2];         // (1/2) w^T Ugam
+    const double2* twx;    // [Mx] exp(-2 pi i k/Mx)
+    const double2* twz;    // [Mz]
+    // workspace
+    double2 *vt, *et;      // state at time t
+    double2* vs;           // v of the current stage (transform input)
+    double2 *uh, *wh, *duh, *dwh;   // u, w, du/dy, dw/dy of the current stage
+    double2* Nh;           // 3 fields: (u.grad)u, (u.grad)v, (u.grad)w in spectral space
+    double2 *F0, *G0, *F1, *G1;     // stored nonlinear terms of stages 0 and 1
+    double2* I8;           // 8 mixed-space fields: u v w Du Dw uz vz wz
+    double2* I3;           // 3 mixed-space fields: Nu Nv Nw
+    double2* uvpart;       // [Ny][Mz][E] (sum_x u v, sum_x w v) per z line
+    double2 *uvc0, *uvc1;  // [Ny][E] plane means of stages 0 and 1
+    double *Ut, *Wt, *Us, *Ws;      // mean profiles at t and at the current stage
+    double *gamma, *Qstar; // [E]
+    double* diag;          // [E][6] + scratch [Ny][E]
+    double2* stage_io;     // staging for ABI-layout copies: 2 spectral fields
+    size_t S;              // Ny*P*E
+    size_t Isz;            // Ny*Mz*nkx*E
+};
+
+struct dns_plan {
+    DnsDev d{};
+    double Lx = 0, Lz = 0;
+    int R1x = 0, R2x = 0, R1z = 0, R2z = 0;   // four-step factorisations of Mx, Mz
+    int ETy = 0;                               // member tile of the per-pair kernel
+    int ETf = 0;                               // member tile of the transform kernels
+    std::vector<void*> owned;                  // plan-owned device allocations
+    void* workspace = nullptr;
+    size_t workspace_bytes = 0;
+    cudaStream_t stream = nullptr;
+    bool bound = false, has_state = false;
+    int sticky = DNS_OK;
+    long long nsteps_done = 0;
+    cudaEvent_t ev[2 * 16] = {};
+    bool ev_init = false;
+};
+
+// host precompute (plan.cu)
+int dns_host_precompute(dns_plan* p);
+bool dns_factor_len(int M, int* R1, int* R2);
+
+// kernel launchers (kernels_*.cu); stage = 0,1,2
+void launch_zinv(dns_plan* p, const double2* vin);
+void launch_line(dns_plan* p);
+void launch_zfwd(dns_plan* p);
+void launch_ypair(dns_plan* p, int stage, int derive_only);
+void launch_mean(dns_plan* p, int stage, int derive_only);
+void launch_abi_to_internal(dns_plan* p, const double2* src_abi, double2* dst);
+void launch_internal_to_abi(dns_plan* p, const double2* src, double2* dst_abi);
+void launch_mean_in(dns_plan* p, const double* U_abi, const double* W_abi);
+void launch_mean_out(dns_plan* p, double* U_abi, double* W_abi);
+void launch_normalise_state(dns_plan* p);
+void launch_diag(dns_plan* p, double t);
