@@ -1,0 +1,273 @@
+"""GPU parity: the CUDA library (through the C ABI binding) against the CPU oracle, element by element on the
+same seeded inputs.  Tolerances are BASELINE.json's: relative 1e-10 in every spectral coefficient after 1 step,
+1e-8 after 20 steps, where "relative" is the reading A14 of DESIGN.md: |a_gpu - a_or| <= tol * s, s = the
+max-modulus of that field of that member.  At the full BASELINE sizes the GPU advances every member and the oracle
+a fixed subset (members are independent, pin P12).  Run with `pytest -m gpu` on a B200.
+"""
+import numpy as np
+import pytest
+
+from oracle.dns_oracle import Oracle
+from paper_2306_12739_b200 import binding, inputs
+
+pytestmark = pytest.mark.gpu
+TOL_1, TOL_20 = 1e-10, 1e-8
+PI = np.pi
+
+
+def field_err(a, b):
+    """max over members of  max|a-b| / max|b|  (per member, per field)."""
+    E = b.shape[0]
+    num = np.abs(a - b).reshape(E, -1).max(axis=1)
+    den = np.abs(b).reshape(E, -1).max(axis=1)
+    den = np.where(den == 0, 1.0, den)
+    return float((num / den).max())
+
+
+def run_pair(cfg, members, steps, check_at=(1,), tol=None, zero_pert=False):
+    """GPU on all cfg.E members, oracle on `members`; returns the errors at the requested step counts."""
+    plan = binding.Plan(*inputs.plan_args(cfg))
+    full = inputs.make_state(cfg)
+    s = 0.0 if zero_pert else 1.0
+    plan.set_state(s * full["vhat"], s * full["etahat"], full["U00"], full["W00"])
+    o = Oracle(*inputs.plan_args(cfg, E=len(members)))
+    idx = list(members)
+    o.set_state(s * full["vhat"][idx], s * full["etahat"][idx], full["U00"][idx], full["W00"][idx])
+    out = {}
+    done = 0
+    for n in sorted(check_at):
+        plan.step(n - done)
+        o.step(n - done)
+        done = n
+        v, eta, U, W = plan.get_state()
+        dg, do = plan.diagnostics()[idx], o.diagnostics()
+        out[n] = dict(v=field_err(v[idx], o.v), eta=field_err(eta[idx], o.eta), U=field_err(U[idx], o.U),
+                      W=float(np.abs(W[idx] - o.W).max() / max(np.abs(o.U).max(), 1e-300)),
+                      diag=float(np.abs(dg - do).max()))
+    plan.close()
+    return out, plan, o
+
+
+def assert_errs(errs, n, tol):
+    e = errs[n]
+    assert e["v"] < tol and e["eta"] < tol and e["U"] < tol and e["W"] < tol, (n, e)
+    assert e["diag"] < 100 * tol, (n, e)
+
+
+# ------------------------------------------------------------------------------------------------ BASELINE configs
+def test_config1_all_members_1_and_20_steps():
+    cfg = inputs.CONFIGS[1]
+    errs, _, _ = run_pair(cfg, range(cfg.E), 20, check_at=(1, 20))
+    assert_errs(errs, 1, TOL_1)
+    assert_errs(errs, 20, TOL_20)
+
+
+def test_config2_sampled_members_1_and_20_steps():
+    cfg = inputs.CONFIGS[2]                       # E = 64: the configuration bench.py times
+    errs, _, _ = run_pair(cfg, [0, 17, 63], 20, check_at=(1, 20))
+    assert_errs(errs, 1, TOL_1)
+    assert_errs(errs, 20, TOL_20)
+
+
+def test_config3_sampled_members_1_and_20_steps():
+    cfg = inputs.CONFIGS[3]                       # Poiseuille, constant mass flux, 64 x 97 x 64, E = 16
+    errs, _, _ = run_pair(cfg, [0, 15], 20, check_at=(1, 20))
+    assert_errs(errs, 1, TOL_1)
+    assert_errs(errs, 20, TOL_20)
+
+
+def test_config4_sampled_members_1_and_20_steps():
+    cfg = inputs.CONFIGS[4]                       # E = 256, per-member amplitudes
+    errs, _, _ = run_pair(cfg, [3, 200], 20, check_at=(1, 20))
+    assert_errs(errs, 1, TOL_1)
+    assert_errs(errs, 20, TOL_20)
+
+
+@pytest.mark.parametrize("E", inputs.SWEEP_E)
+def test_config5_sweep_one_step(E):
+    cfg = inputs.CONFIGS[5].with_E(E)
+    members = sorted({0, E - 1})
+    errs, _, _ = run_pair(cfg, members, 1)
+    assert_errs(errs, 1, TOL_1)
+
+
+# ------------------------------------------------------------------------------------------------ edge cases
+@pytest.mark.parametrize("Nx,Nz", [(12, 16), (16, 12), (18, 24), (24, 18), (32, 36), (36, 32), (48, 54), (54, 48),
+                                   (64, 72), (72, 64)])
+def test_every_transform_length_both_directions(Nx, Nz):
+    """All 3N/2 = 2^a 3^b lengths in 16..128 (18..108), as x and as z length; ragged member tile E = 3."""
+    cfg = inputs.Config(1, inputs.COUETTE, 350.0, 1.9 * PI, 1.1 * PI, Nx, 13, Nz, 3, 0.01, 1, 0.1, 0, box=3)
+    errs, _, _ = run_pair(cfg, range(3), 2, check_at=(1, 2))
+    assert_errs(errs, 1, TOL_1)
+    assert_errs(errs, 2, TOL_1 * 10)
+
+
+@pytest.mark.parametrize("E,Ny,flow", [(1, 17, 0), (5, 20, 1), (33, 12, 0), (7, 5, 1), (2, 66, 1)])
+def test_ragged_members_and_odd_even_ny(E, Ny, flow):
+    cfg = inputs.Config(3 if flow else 1, flow, 500.0, 2 * PI, PI, 16, Ny, 12, E, 0.01, 1, 0.1, 0, box=2)
+    errs, _, _ = run_pair(cfg, range(E), 3, check_at=(1, 3))
+    assert_errs(errs, 1, TOL_1)
+    assert_errs(errs, 3, TOL_1 * 10)
+
+
+def test_laminar_fixed_points_on_gpu_at_full_size():
+    for cid, prof in ((2, lambda y: y), (3, lambda y: 1.5 * (1 - y * y))):
+        cfg = inputs.CONFIGS[cid]
+        plan = binding.Plan(*inputs.plan_args(cfg))
+        st = inputs.make_state(cfg)
+        plan.set_state(0 * st["vhat"], 0 * st["etahat"], st["U00"], st["W00"])
+        plan.step(5)
+        v, eta, U, W = plan.get_state()
+        y = inputs.grid_y(cfg.Ny)
+        assert np.abs(U - prof(y)).max() < 1e-13 and np.abs(v).max() == 0 and np.abs(eta).max() == 0
+        d = plan.diagnostics()
+        if cid == 3:
+            assert np.abs(d[:, 4] - 3.0 / cfg.Re).max() < 1e-15 * cfg.Re     # gamma = 2c/Re, c = 1.5
+            assert np.abs(d[:, 3] - 1.0).max() < 1e-13
+        plan.close()
+
+
+def test_flux_conservation_and_noslip_at_full_size():
+    cfg = inputs.CONFIGS[3]
+    plan = binding.Plan(*inputs.plan_args(cfg))
+    st = inputs.make_state(cfg)
+    plan.set_state(st["vhat"], st["etahat"], st["U00"], st["W00"])
+    q0 = plan.diagnostics()[:, 3]
+    plan.step(10)
+    d = plan.diagnostics()
+    assert np.abs(d[:, 3] - q0).max() < 1e-13                                 # pin P5 on the GPU
+    v, eta, U, W = plan.get_state()
+    assert np.all(v[..., 0] == 0) and np.all(v[..., -1] == 0) and np.all(eta[..., 0] == 0)
+    assert np.all(v[:, 0, 0] == 0) and np.all(eta[:, 0, 0] == 0)
+    assert np.all(U[:, 0] == 0) and np.all(U[:, -1] == 0) and np.all(W[:, 0] == 0)
+    assert np.all(np.isfinite(d))
+    plan.close()
+
+
+def test_member_independence_bitwise():
+    """P12 on the GPU: a member's result does not depend on E or on the other members."""
+    cfg5 = inputs.CONFIGS[1].with_E(5)
+    full = inputs.make_state(cfg5)
+    plan = binding.Plan(*inputs.plan_args(cfg5))
+    plan.set_state(full["vhat"], full["etahat"], full["U00"], full["W00"])
+    plan.step(3)
+    v5, e5, U5, W5 = plan.get_state()
+    plan.close()
+    idx = [4, 1]
+    plan2 = binding.Plan(*inputs.plan_args(cfg5, E=2))
+    plan2.set_state(full["vhat"][idx], full["etahat"][idx], full["U00"][idx], full["W00"][idx])
+    plan2.step(3)
+    v2, e2, U2, W2 = plan2.get_state()
+    plan2.close()
+    assert np.array_equal(v2, v5[idx]) and np.array_equal(e2, e5[idx]) and np.array_equal(U2, U5[idx])
+
+
+def test_step_n_equals_n_steps_and_is_deterministic():
+    cfg = inputs.CONFIGS[1]
+    st = inputs.make_state(cfg)
+    res = []
+    for chunks in ((4,), (1, 1, 2), (4,)):
+        plan = binding.Plan(*inputs.plan_args(cfg))
+        plan.set_state(st["vhat"], st["etahat"], st["U00"], st["W00"])
+        for c in chunks:
+            plan.step(c)
+        res.append(plan.get_state())
+        assert plan.diagnostics()[0, 5] == pytest.approx(4 * cfg.dt)
+        plan.close()
+    for r in res[1:]:
+        for a, b in zip(r, res[0]):
+            assert np.array_equal(a, b)
+
+
+def test_set_state_normalisation_matches_oracle():
+    cfg = inputs.CONFIGS[1]
+    st = inputs.make_state(cfg)
+    rng = np.random.default_rng(7)
+    v = st["vhat"] + 0.01 * (rng.standard_normal(st["vhat"].shape) + 1j * rng.standard_normal(st["vhat"].shape))
+    eta = st["etahat"] + 0.01 * rng.standard_normal(st["vhat"].shape)
+    U = st["U00"] + 0.3
+    W = st["W00"] + 0.1
+    plan = binding.Plan(*inputs.plan_args(cfg))
+    plan.set_state(v, eta, U, W)
+    o = Oracle(*inputs.plan_args(cfg))
+    o.set_state(v, eta, U, W)
+    gv, ge, gU, gW = plan.get_state()
+    assert np.array_equal(gv, o.v) and np.array_equal(ge, o.eta) and np.array_equal(gU, o.U) and np.array_equal(gW, o.W)
+    plan.step(1)
+    o.step(1)
+    gv, ge, gU, gW = plan.get_state()
+    assert field_err(gv, o.v) < TOL_1 and field_err(ge, o.eta) < TOL_1 and field_err(gU, o.U) < TOL_1
+    plan.close()
+
+
+def test_device_pointer_io():
+    import torch
+    cfg = inputs.CONFIGS[1]
+    st = inputs.make_state(cfg)
+    plan = binding.Plan(*inputs.plan_args(cfg))
+    dev = [torch.from_numpy(np.ascontiguousarray(st[k])).cuda() for k in ("vhat", "etahat", "U00", "W00")]
+    plan.set_state(*dev)
+    plan.step(2)
+    outs = [torch.empty_like(t) for t in dev]
+    plan.get_state(outs)
+    plan2 = binding.Plan(*inputs.plan_args(cfg))
+    plan2.set_state(st["vhat"], st["etahat"], st["U00"], st["W00"])
+    plan2.step(2)
+    host = plan2.get_state()
+    for a, b in zip(outs, host):
+        assert np.array_equal(a.cpu().numpy(), b)
+    plan.close()
+    plan2.close()
+
+
+def test_error_paths_on_device():
+    cfg = inputs.CONFIGS[1]
+    st, h = binding.dns_plan_create(*inputs.plan_args(cfg))
+    assert st == binding.DNS_OK
+    assert binding.dns_step(h, 1) == binding.DNS_ESTATE                      # nothing bound
+    import torch
+    n = binding.dns_plan_workspace_bytes(h)
+    assert n > 0
+    small = torch.empty(1024, dtype=torch.uint8, device="cuda")
+    assert binding.dns_plan_bind(h, small.data_ptr(), 1024) == binding.DNS_EINVAL
+    ws = torch.empty(n + 256, dtype=torch.uint8, device="cuda")
+    base = (ws.data_ptr() + 255) & ~255
+    assert binding.dns_plan_bind(h, base + 8, n) == binding.DNS_EINVAL       # misaligned
+    assert binding.dns_plan_bind(h, base, n) == binding.DNS_OK
+    assert binding.dns_step(h, 1) == binding.DNS_ESTATE                      # no state yet
+    assert binding.dns_step(h, -1) == binding.DNS_EINVAL
+    assert binding.dns_launches_per_step(h) > 0
+    assert binding.dns_plan_destroy(h) == binding.DNS_OK
+
+
+def test_nonfinite_energy_is_reported():
+    cfg = inputs.CONFIGS[1]
+    st = inputs.make_state(cfg)
+    v = st["vhat"].copy()
+    v[1, 2, 3, 5] = np.nan
+    plan = binding.Plan(*inputs.plan_args(cfg))
+    plan.set_state(v, st["etahat"], st["U00"], st["W00"])
+    out = np.empty((cfg.E, 6))
+    assert binding.dns_diagnostics(plan.h, out) == binding.DNS_ENONFINITE
+    assert np.isfinite(out[0, 0]) and not np.isfinite(out[1, 0])
+    plan.close()
+
+
+def test_stage_pieces_against_oracle():
+    """Per-kernel parity through the debug hook: reconstruction (Eq. 17-18), the spectral advection terms and
+    F^0, G^0 (Eq. 4-5) of the first stage."""
+    cfg = inputs.CONFIGS[2].with_E(5)
+    st = inputs.make_state(cfg)
+    plan = binding.Plan(*inputs.plan_args(cfg))
+    plan.set_state(st["vhat"], st["etahat"], st["U00"], st["W00"])
+    o = Oracle(*inputs.plan_args(cfg))
+    o.set_state(st["vhat"], st["etahat"], st["U00"], st["W00"])
+    u, v, w, Du, Dv, Dw = o.velocities(o.v, o.eta, o.U, o.W)
+    for which, ref in ((0, u), (1, w), (2, Du), (3, Dw)):
+        got = plan.debug_fetch(which)
+        assert field_err(got[..., 1:-1], ref[..., 1:-1]) < 1e-12, which
+    F, G, Su, Sw = o.nonlinear(o.v, o.eta, o.U, o.W)
+    plan.step(1)
+    assert field_err(plan.debug_fetch(5)[..., 1:-1], F) < 1e-11
+    assert field_err(plan.debug_fetch(6)[..., 1:-1], G) < 1e-11
+    plan.close()
