@@ -8,7 +8,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libdns_b200.so")
-SOURCES = ["api.cu", "plan.cu", "kernels_fft.cu", "kernels_y.cu"]
+SOURCES = ["api.cu", "plan.cu", "kernels_fft.cu", "kernels_line.cu", "kernels_y.cu"]
 HEADERS = ["dns_internal.h", "fft_codelets.cuh", "fft_consts.h", os.path.join("..", "..", "include", "dns.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "--expt-relaxed-constexpr",
