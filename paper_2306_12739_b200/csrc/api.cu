@@ -117,7 +117,14 @@ int dns_plan_create(dns_plan** out, int Nx, int Ny, int Nz, int E, double Re, do
     d.nkx = Nx / 2; d.nkz = Nz - 1; d.nzh = Nz / 2; d.P = d.nkx * d.nkz; d.Ni = Ny - 2; d.flow = flow;
     d.dt = dt; d.Re = Re; d.Uw = flow == DNS_COUETTE ? 1.0 : 0.0; d.invMxMz = 1.0 / ((double)Mx * Mz);
     d.S = (size_t)Ny * d.P * E;
-    d.Isz = (size_t)Ny * Mz * d.nkx * E;
+    {
+        const int tps = dns_line_tps(Mx);                // lanes per slot of the line kernel = largest member tile
+        int et = 1, lg = 0;
+        while (et < tps && et < E) { et <<= 1; ++lg; }
+        d.etl = lg;
+        d.ntl = (E + et - 1) / et;
+        d.Isz = ((size_t)Ny * Mz * d.ntl * d.nkx) << lg;
+    }
     p->Lx = Lx; p->Lz = Lz;
     // member tiles
     p->ETf = pow2ceil(E) < 32 ? pow2ceil(E) : 32;

@@ -8,9 +8,11 @@
 
 // Everything a kernel needs, passed by value.  Spectral arrays are [Ny][nkx][nkz][E] complex (member index
 // fastest: the paper's vectorised-ensemble axis, is the coalescing axis); mixed (kx, z) arrays
-// are [Ny][Mz][nkx][E] complex; mean-flow arrays are [Ny][E] real.
+// are [Ny][Mz][ntl][nkx][2^etl] complex (member tiles, so that one (line, tile) block of a field is contiguous:
+// one TMA bulk copy in the line kernel); mean-flow arrays are [Ny][E] real.
 struct DnsDev {
     int Nx, Ny, Nz, E, Mx, Mz, nkx, nkz, nzh, P, Ni, flow;
+    int etl, ntl;          // mixed arrays are tile-major: member tile of 2^etl lanes, ntl = ceil(E / 2^etl) tiles
     double dt, Re, Uw, invMxMz;
     // plan-owned constant tables
     const double* kx;      // [nkx]
@@ -40,8 +42,13 @@ struct DnsDev {
     double* diag;          // [E][6] + scratch [Ny][E]
     double2* stage_io;     // staging for ABI-layout copies: 2 spectral fields
     size_t S;              // Ny*P*E
-    size_t Isz;            // Ny*Mz*nkx*E
+    size_t Isz;            // Ny*Mz*ntl*nkx*2^etl
 };
+
+// offset of element (plane j, line q, mode n, member e) inside one mixed field
+__host__ __device__ inline size_t dns_mix_off(const DnsDev& d, int j, int q, int n, int e) {
+    return ((((((size_t)j * d.Mz + q) * d.ntl + (e >> d.etl)) * d.nkx + n) << d.etl)) + (e & ((1 << d.etl) - 1));
+}
 
 struct dns_plan {
     DnsDev d{};
@@ -49,6 +56,7 @@ struct dns_plan {
     int R1x = 0, R2x = 0, R1z = 0, R2z = 0;   // four-step factorisations of Mx, Mz
     int ETy = 0;                               // member tile of the per-pair kernel
     int ETf = 0;                               // member tile of the transform kernels
+    int line_grid = 0;                         // persistent grid of the line kernel (set at first launch)
     std::vector<void*> owned;                  // plan-owned device allocations
     void* workspace = nullptr;
     size_t workspace_bytes = 0;
@@ -63,6 +71,7 @@ struct dns_plan {
 // host precompute (plan.cu)
 int dns_host_precompute(dns_plan* p);
 bool dns_factor_len(int M, int* R1, int* R2);
+int dns_line_tps(int Mx);
 
 // kernel launchers (kernels_*.cu); stage = 0,1,2
 void launch_zinv(dns_plan* p, const double2* vin);

@@ -82,9 +82,10 @@ __global__ void __launch_bounds__(256) k_zinv(DnsDev d, const double2* __restric
         DFT<R1>::run(x);
         if (n < d.nkx && eok) {
             const int fo = var ? 5 + f : f;
-            double2* dst = d.I8 + (((size_t)fo * d.Ny + j) * d.Mz) * d.nkx * d.E + (size_t)n * d.E + e;
+            double2* dst = d.I8 + (size_t)fo * d.Isz + dns_mix_off(d, j, 0, n, e);
+            const size_t qs = ((size_t)d.ntl * d.nkx) << d.etl;
 #pragma unroll
-            for (int k1 = 0; k1 < R1; ++k1) dst[(size_t)(k2 + R2 * k1) * d.nkx * d.E] = cswap(x[k1]);
+            for (int k1 = 0; k1 < R1; ++k1) dst[(size_t)(k2 + R2 * k1) * qs] = cswap(x[k1]);
         }
     }
 }
@@ -111,10 +112,12 @@ __global__ void __launch_bounds__(256) k_zfwd(DnsDev d, int etlog, int NB) {
     for (int item = slot; item < NB * R1; item += nslots) {
         const int nb = item / R1, i1 = item % R1, n = n0 + nb;
         double2 a[R2];
-        const double2* src = d.I3 + (((size_t)f * d.Ny + j) * d.Mz) * d.nkx * d.E + (size_t)n * d.E + e;
+        const bool ok = n < d.nkx && eok;
+        const double2* src = d.I3 + (size_t)f * d.Isz + dns_mix_off(d, j, 0, ok ? n : 0, ok ? e : 0);
+        const size_t qs = ((size_t)d.ntl * d.nkx) << d.etl;
 #pragma unroll
         for (int i2 = 0; i2 < R2; ++i2)
-            a[i2] = (n < d.nkx && eok) ? src[(size_t)(i1 + R1 * i2) * d.nkx * d.E] : make_double2(0.0, 0.0);
+            a[i2] = ok ? src[(size_t)(i1 + R1 * i2) * qs] : make_double2(0.0, 0.0);
         DFT<R2>::run(a);
 #pragma unroll
         for (int k2 = 0; k2 < R2; ++k2) buf[((size_t)nb * M + i1 * R2 + k2) * ET + e_l] = cmul(a[k2], tws[i1 * k2]);

@@ -1,6 +1,6 @@
 // Fused x-line kernel (SURVEY.md 8(a) rows a4 (x part), a5, a6 (x part); north_star subsystems (1) and (2)).
 // One "line" = (plane j, z index q, member e).  For every line the kernel
-//   * reads the 8 mixed (kx, z) fields u v w Du Dw uz vz wz written by k_zinv, each exactly once per retained kx,
+//   * reads the 8 mixed (kx, z) fields u v w Du Dw uz vz wz written by k_zinv, each exactly once,
 //   * forms the 11 physical fields u, v, w, their x/z derivatives and Du, Dw with 6 Hermitian two-for-one complex
 //     inverse FFTs along x (x-derivatives = i kx folded into the packing; dv/dy = -du/dx - dw/dz pointwise, which
 //     holds exactly at interior rows for the u, w of Eq. 17-18),
@@ -9,8 +9,13 @@
 // Nothing in physical space ever reaches HBM.
 //
 // Thread mapping: a line is shared by SL "slots"; every slot owns R1 x-points of each physical field in registers.
-// A CTA is one group of SL slots x TPS lanes (lanes = members, or members x lines when E < TPS), 32..96 threads,
-// so the four-step exchanges need only a warp- or CTA-local barrier and many independent groups are resident per SM.
+// A "group" = SL slots x TPS lanes (lanes = members, or members x lines when E < TPS) = 1..3 warps; the four-step
+// exchanges need only a group-local barrier.  Groups are persistent: each walks over work items (j, q-group, member
+// tile).  The mixed arrays are stored tile-major ([j][q][tile][kx][ET]) so that the input of one item and one field
+// is ONE contiguous block, fetched by a single TMA bulk copy (cp.async.bulk + mbarrier) into a ring of field slots
+// one item ahead of the arithmetic: global latency never touches the register file or the LSU pipe.
+#include <cstdint>
+
 #include "dns_internal.h"
 #include "fft_codelets.cuh"
 
@@ -18,8 +23,33 @@ using namespace dnsfft;
 
 namespace {
 
-template <int BT> __device__ __forceinline__ void group_sync() {
-    if (BT == 32) __syncwarp(); else __syncthreads();
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred P1;\n"
+        "LAB_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+        "@P1 bra DONE;\n"
+        "bra LAB_WAIT;\n"
+        "DONE:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+
+template <int GT> __device__ __forceinline__ void group_sync(int grp) {
+    if (GT == 32) __syncwarp();
+    else asm volatile("bar.sync %0, %1;" ::"r"(grp + 1), "r"(GT) : "memory");
 }
 
 // row pitch (in double2) of an exchange buffer with `cols` columns of TPS lanes: for TPS = 4 two slots share a
@@ -28,130 +58,182 @@ constexpr int line_pitch(int cols, int TPS) {
     return TPS >= 8 ? cols * TPS : cols * TPS + ((TPS - (cols * TPS) % 8 + 8) % 8);
 }
 
-// mode index loaded for padded position pos: n (positive side), M - pos (negative side, conjugated) or -1 (zero)
+// mode index read for padded position pos: n (positive side), M - pos (negative side, conjugated) or -1 (zero)
 template <int M, int NKX> __device__ __forceinline__ int pos_mode(int pos) {
     return pos < NKX ? pos : (pos > M - NKX ? M - pos : -1);
 }
 
-// Field pairing of the six complex transforms Z = A + iB (A, B real in x):
-//   C = 0: (v, dv/dx)   1: (u, du/dx)   2: (w, dw/dx)   3: (Du, du/dz)   4: (Dw, dw/dz)   5: (dv/dz, -)
-// I8 field order: 0 u, 1 v, 2 w, 3 Du, 4 Dw, 5 uz, 6 vz, 7 wz.
-template <int C> struct LinePair;
-template <> struct LinePair<0> { static constexpr int fa = 1, fb = -1; };
-template <> struct LinePair<1> { static constexpr int fa = 0, fb = -1; };
-template <> struct LinePair<2> { static constexpr int fa = 2, fb = -1; };
-template <> struct LinePair<3> { static constexpr int fa = 3, fb = 5; };
-template <> struct LinePair<4> { static constexpr int fa = 4, fb = 7; };
-template <> struct LinePair<5> { static constexpr int fa = 6, fb = -1; };
-
-template <int C, int R1, int R2>
-__device__ __forceinline__ void line_load(const double2* __restrict__ src, size_t fstride, int E, int sl, bool act,
-                                          double2 (&ra)[R2], double2 (&rb)[R2]) {
-    constexpr int M = R1 * R2, NKX = M / 3;
-#pragma unroll
-    for (int i2 = 0; i2 < R2; ++i2) {
-        const int lo = R1 * i2, hi = R1 * i2 + R1 - 1;
-        if (lo >= NKX && hi <= M - NKX) continue;               // statically zero padding
-        const int n = pos_mode<M, NKX>(sl + R1 * i2);
-        ra[i2] = make_double2(0.0, 0.0);
-        if (LinePair<C>::fb >= 0) rb[i2] = make_double2(0.0, 0.0);
-        if (act && n >= 0) {
-            ra[i2] = __ldg(src + (size_t)LinePair<C>::fa * fstride + (size_t)n * E);
-            if (LinePair<C>::fb >= 0) rb[i2] = __ldg(src + (size_t)LinePair<C>::fb * fstride + (size_t)n * E);
-        }
-    }
+// Order in which the 8 mixed fields are consumed (sequence s -> field of I8: 0 u, 1 v, 2 w, 3 Du, 4 Dw, 5 uz, 6 vz,
+// 7 wz) by the six complex transforms Z = A + iB (A, B real in x):
+//   C = 0: (v, dv/dx)  1: (u, du/dx)  2: (w, dw/dx)  3: (Du, du/dz)  4: (Dw, dw/dz)  5: (dv/dz, -)
+__device__ __forceinline__ constexpr int seq_field(int s) {
+    return s == 0 ? 1 : s == 1 ? 0 : s == 2 ? 2 : s == 3 ? 3 : s == 4 ? 5 : s == 5 ? 4 : s == 6 ? 7 : 6;
 }
+template <int C> struct LineSeq { static constexpr int sa = C < 3 ? C : (C == 3 ? 3 : (C == 4 ? 5 : 7)), two = (C == 3 || C == 4); };
 
-// inverse pass A: pack Z(pos), R2-point DFTs over pos = sl + R1*i2, twiddle, store row sl
-template <int C, int R1, int R2, int TPS>
-__device__ __forceinline__ void line_pass_a(const double2 (&ra)[R2], const double2 (&rb)[R2], const double* kxs,
-                                            const double2* tws, double2* buf, int sl, int lis) {
-    constexpr int M = R1 * R2, NKX = M / 3, PI = line_pitch(R2, TPS);
-    double2 a[R2];
-#pragma unroll
-    for (int i2 = 0; i2 < R2; ++i2) {
-        const int lo = R1 * i2, hi = R1 * i2 + R1 - 1;
-        if (lo >= NKX && hi <= M - NKX) { a[i2] = make_double2(0.0, 0.0); continue; }
-        const int pos = sl + R1 * i2;
-        const int n = pos_mode<M, NKX>(pos);
-        const bool neg = pos >= NKX;
-        const double2 A = ra[i2];
-        double2 z;
-        if (LinePair<C>::fb >= 0) {
-            const double2 B = rb[i2];
-            // Z(n) = A + iB ; Z(0) = (Re A, Re B) ; Z(M - n) = conj(A) + i conj(B)
-            z = neg ? make_double2(A.x + B.y, B.x - A.y)
-                    : (pos == 0 ? make_double2(A.x, B.x) : make_double2(A.x - B.y, A.y + B.x));
-        } else if (C < 3) {
-            // B = i kx A:  Z(n) = (1 - kx) A ; Z(M - n) = (1 + kx) conj(A)
-            const double kx = n >= 0 ? kxs[n] : 0.0;
-            z = neg ? make_double2((1.0 + kx) * A.x, -(1.0 + kx) * A.y)
-                    : (pos == 0 ? make_double2(A.x, 0.0) : make_double2((1.0 - kx) * A.x, (1.0 - kx) * A.y));
-        } else {
-            z = neg ? make_double2(A.x, -A.y) : (pos == 0 ? make_double2(A.x, 0.0) : A);
-        }
-        a[i2] = cswap(z);                                       // inverse transform by the swap identity
-    }
-    DFT<R2>::run(a);
-#pragma unroll
-    for (int k2 = 0; k2 < R2; ++k2) buf[sl * PI + k2 * TPS + lis] = cmul(a[k2], tws[sl * k2]);
+struct LineSmem {                     // byte offsets inside the dynamic shared memory of a CTA
+    int tws_i, tws_f, kxs, group0, group_bytes, ring, buf, exch, red, bars, total;
+};
+__host__ __device__ inline LineSmem line_smem(int R1, int R2, int SL, int TPS, int NG, int NST) {
+    const int M = R1 * R2, NKX = M / 3;
+    const int PI = line_pitch(R2, TPS), PF = line_pitch(R1, TPS);
+    const int BUF = (R1 * PI > R2 * PF) ? R1 * PI : R2 * PF;
+    LineSmem s{};
+    int off = 0;
+    auto take = [&](int bytes) { int o = off; off += (bytes + 127) & ~127; return o; };
+    s.tws_i = take(R2 * SL * 16);
+    s.tws_f = take(R1 * SL * 16);
+    s.kxs = take(NKX * 8);
+    s.group0 = off;
+    off = 0;
+    s.ring = take(NST * NKX * TPS * 16);
+    s.buf = take(2 * BUF * 16);
+    s.exch = take(NKX * TPS * 16);
+    s.red = take(SL * TPS * 16);
+    s.bars = take(NST * 8);
+    s.group_bytes = off;
+    s.total = s.group0 + NG * s.group_bytes;
+    return s;
 }
 
 // ------------------------------------------------------------------------------------------------ the kernel
-// grid = Ni * nblk_q * ntile_e ; block = SL * TPS
-template <int R1, int R2, int SL, int TPS, int MINB>
-__global__ void __launch_bounds__(SL * TPS, MINB) k_line(DnsDev d, int etlog, int LQ) {
-    constexpr int M = R1 * R2, NKX = M / 3, BT = SL * TPS;
+// grid = persistent CTAs ; block = NG groups of SL * TPS threads
+template <int R1, int R2, int SL, int TPS, int NG, int NST, int MINB>
+__global__ void __launch_bounds__(SL * TPS * NG, MINB) k_line(DnsDev d, int nitems) {
+    constexpr int M = R1 * R2, NKX = M / 3, GT = SL * TPS;
     constexpr int PI = line_pitch(R2, TPS), PF = line_pitch(R1, TPS);
     constexpr int BUF = (R1 * PI > R2 * PF) ? R1 * PI : R2 * PF;
-    __shared__ double2 tws[M];
-    __shared__ double kxs[NKX];
-    __shared__ double2 buf[2][BUF];
-    __shared__ double2 exch[NKX * TPS];
-    __shared__ double2 red[SL * TPS];
+    constexpr int SLOT = NKX * TPS;                          // double2 per ring slot
+    static_assert(NST == 8 || NST == 4, "ring depth");
+    extern __shared__ __align__(128) unsigned char smraw[];
+    const LineSmem L = line_smem(R1, R2, SL, TPS, NG, NST);
+    double2* tws_i = reinterpret_cast<double2*>(smraw + L.tws_i);      // [k2][slot] = w_M^(slot k2)
+    double2* tws_f = reinterpret_cast<double2*>(smraw + L.tws_f);      // [k][slot]
+    double* kxs = reinterpret_cast<double*>(smraw + L.kxs);
+    const int grp = threadIdx.x / GT, t = threadIdx.x % GT;
+    unsigned char* gs = smraw + L.group0 + grp * L.group_bytes;
+    double2* ring = reinterpret_cast<double2*>(gs + L.ring);
+    double2* buf0 = reinterpret_cast<double2*>(gs + L.buf);
+    double2* buf1 = buf0 + BUF;
+    double2* exch = reinterpret_cast<double2*>(gs + L.exch);
+    double2* red = reinterpret_cast<double2*>(gs + L.red);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(gs + L.bars);
 
-    const int t = threadIdx.x, sl = t / TPS, lis = t % TPS;
-    const int ET = 1 << etlog, el = lis & (ET - 1), lc = lis >> etlog, LC = TPS >> etlog;
-    const int ntile_e = (d.E + ET - 1) >> etlog, nblk_q = (d.Mz + LC * LQ - 1) / (LC * LQ);
-    int b = blockIdx.x;
-    const int te = b % ntile_e; b /= ntile_e;
-    const int bq = b % nblk_q;  b /= nblk_q;
-    const int j = b + 1;                                    // interior planes only (wall planes give N = 0 exactly)
-    const int e = te * ET + el;
-    const bool eok = e < d.E;
-    for (int i = t; i < M; i += BT) tws[i] = d.twx[i];
-    for (int i = t; i < NKX; i += BT) kxs[i] = d.kx[i];
+    const int sl = t / TPS, lis = t % TPS;
+    const int etlog = d.etl, ET = 1 << etlog, el = lis & (ET - 1), lc = lis >> etlog, LC = TPS >> etlog;
+    const int ntile = d.ntl, nqg = (d.Mz + LC - 1) / LC;
+    for (int i = threadIdx.x; i < R2 * SL; i += blockDim.x) tws_i[i] = d.twx[((i % SL) * (i / SL)) % M];
+    for (int i = threadIdx.x; i < R1 * SL; i += blockDim.x) tws_f[i] = d.twx[((i % SL) * (i / SL)) % M];
+    for (int i = threadIdx.x; i < NKX; i += blockDim.x) kxs[i] = d.kx[i];
+    if (t == 0) {
+        for (int s = 0; s < NST; ++s) mbar_init(bars + s, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
     __syncthreads();
+
     const size_t fstride = d.Isz;
     const int E = d.E;
+    const int stride = gridDim.x * NG;
+    const int lidx = (lc * NKX) * ET + el;                   // + n * ET : element of this lane inside a slot / item block
+    // item -> offset of its block inside one mixed field, number of valid lines
+    auto item_off = [&](int it, int& nl) -> size_t {
+        const int te = it % ntile, qg = (it / ntile) % nqg, jj = it / (ntile * nqg) + 1;
+        nl = d.Mz - qg * LC < LC ? d.Mz - qg * LC : LC;
+        return ((((size_t)jj * d.Mz + (size_t)qg * LC) * ntile + te) * NKX) << etlog;
+    };
+    auto issue = [&](int it, int s) {                         // leader only: fetch sequence s of item it
+        int nl;
+        const size_t off = item_off(it, nl);
+        const uint32_t bytes = (uint32_t)(nl * NKX * ET * 16);
+        uint64_t* bar = bars + (s % NST);
+        mbar_arrive_expect_tx(bar, bytes);
+        bulk_g2s(ring + (s % NST) * SLOT, d.I8 + (size_t)seq_field(s) * fstride + off, bytes, bar);
+    };
 
-    for (int qi = 0; qi < LQ; ++qi) {
-        const int q = (bq * LQ + qi) * LC + lc;
-        const bool lok = eok && q < d.Mz;
-        const size_t base = (((size_t)j * d.Mz + (lok ? q : 0)) * NKX) * E + (eok ? e : 0);
-        const double2* src = d.I8 + base;
-        const bool act = lok && sl < R1;
+    int it = blockIdx.x * NG + grp;
+    if (t == 0 && it < nitems)
+        for (int s = 0; s < NST; ++s) issue(it, s);
+    uint32_t itc = 0;                                        // items done by this group
+
+    for (; it < nitems; it += stride, ++itc) {
+        const int nxt = it + stride;
+        int nl;
+        const size_t ioff = item_off(it, nl);
+        const int te = it % ntile, qg = (it / ntile) % nqg, j = it / (ntile * nqg) + 1;
+        const int q = qg * LC + lc, e = te * ET + el;
+        const bool lok = e < E && lc < nl;
         double u[R1], v[R1], w[R1], Nu[R1], Nv[R1], Nw[R1];
         double suv = 0.0, swv = 0.0;
-        double2 ra[R2], rb[R2];
 
-#define DNS_LINE_INV(C, BODY)                                                              \
-        if (sl < R1) line_pass_a<C, R1, R2, TPS>(ra, rb, kxs, tws, buf[(C) & 1], sl, lis); \
-        group_sync<BT>();                                                                  \
-        if ((C) < 5) line_load<((C) < 5 ? (C) + 1 : 5), R1, R2>(src, fstride, E, sl, act, ra, rb); \
-        if (sl < R2) {                                                                     \
-            double2 x[R1];                                                                 \
-            _Pragma("unroll")                                                              \
-            for (int i1 = 0; i1 < R1; ++i1) x[i1] = buf[(C) & 1][i1 * PI + sl * TPS + lis]; \
-            DFT<R1>::run(x);                                                               \
-            _Pragma("unroll")                                                              \
-            for (int k = 0; k < R1; ++k) {                                                 \
-                const double fa = x[k].y, fb = x[k].x; (void)fb;                           \
-                BODY                                                                       \
-            }                                                                              \
+        // wait for sequence s of this item; refill slot after use with sequence s + NST (this or the next item)
+        auto wait_seq = [&](int s) {
+            const uint32_t use = NST == 8 ? itc : 2 * itc + (s >= 4 ? 1 : 0);
+            mbar_wait(bars + (s % NST), use & 1);
+        };
+        auto refill = [&](int s) {
+            if (t != 0) return;
+            if (NST == 4 && s < 4) issue(it, s + 4);
+            else if (nxt < nitems) issue(nxt, NST == 8 ? s : s - 4);
+        };
+
+#define DNS_LINE_INV(C, BODY)                                                                         \
+        {                                                                                             \
+            constexpr int sa = LineSeq<C>::sa, two = LineSeq<C>::two;                                 \
+            wait_seq(sa);                                                                             \
+            if (two) wait_seq(sa + 1);                                                                \
+            double2* bufc = ((C) & 1) ? buf1 : buf0;                                                  \
+            if (sl < R1) {                                                                            \
+                const double2* fa_s = ring + (sa % NST) * SLOT + lidx;                                \
+                const double2* fb_s = ring + ((sa + 1) % NST) * SLOT + lidx;                          \
+                double2 a[R2];                                                                        \
+                _Pragma("unroll")                                                                     \
+                for (int i2 = 0; i2 < R2; ++i2) {                                                     \
+                    const int lo = R1 * i2, hi = R1 * i2 + R1 - 1;                                    \
+                    if (lo >= NKX && hi <= M - NKX) { a[i2] = make_double2(0.0, 0.0); continue; }     \
+                    const int pos = sl + R1 * i2;                                                     \
+                    const int n = pos_mode<M, NKX>(pos);                                              \
+                    const bool neg = pos >= NKX;                                                      \
+                    double2 z = make_double2(0.0, 0.0);                                               \
+                    if (n >= 0) {                                                                     \
+                        const double2 A = fa_s[n << etlog];                                           \
+                        if (two) {                                                                    \
+                            const double2 B = fb_s[n << etlog];                                       \
+                            z = neg ? make_double2(A.x + B.y, B.x - A.y)                              \
+                                    : (pos == 0 ? make_double2(A.x, B.x) : make_double2(A.x - B.y, A.y + B.x)); \
+                        } else if ((C) < 3) {                                                         \
+                            const double kx = kxs[n];                                                 \
+                            z = neg ? make_double2((1.0 + kx) * A.x, -(1.0 + kx) * A.y)               \
+                                    : (pos == 0 ? make_double2(A.x, 0.0) : make_double2((1.0 - kx) * A.x, (1.0 - kx) * A.y)); \
+                        } else {                                                                      \
+                            z = neg ? make_double2(A.x, -A.y) : (pos == 0 ? make_double2(A.x, 0.0) : A); \
+                        }                                                                             \
+                    }                                                                                 \
+                    a[i2] = cswap(z);                                                                 \
+                }                                                                                     \
+                DFT<R2>::run(a);                                                                      \
+                _Pragma("unroll")                                                                     \
+                for (int k2 = 0; k2 < R2; ++k2) bufc[sl * PI + k2 * TPS + lis] = cmul(a[k2], tws_i[k2 * SL + sl]); \
+            }                                                                                         \
+            group_sync<GT>(grp);                                                                      \
+            refill(sa);                                                                               \
+            if (two) refill(sa + 1);                                                                  \
+            if (sl < R2) {                                                                            \
+                double2 x[R1];                                                                        \
+                _Pragma("unroll")                                                                     \
+                for (int i1 = 0; i1 < R1; ++i1) x[i1] = bufc[i1 * PI + sl * TPS + lis];               \
+                DFT<R1>::run(x);                                                                      \
+                _Pragma("unroll")                                                                     \
+                for (int k = 0; k < R1; ++k) {                                                        \
+                    const double fa = x[k].y, fb = x[k].x; (void)fb;                                  \
+                    BODY                                                                              \
+                }                                                                                     \
+            }                                                                                         \
         }
 
-        line_load<0, R1, R2>(src, fstride, E, sl, act, ra, rb);
+        // Z = A + iB:  Z(n) = A + iB, Z(0) = (Re A, Re B), Z(M - n) = conj(A) + i conj(B); with B = i kx A this is
+        // Z(n) = (1 - kx) A, Z(M - n) = (1 + kx) conj(A).  Inverse transform by the swap identity: after the two
+        // passes the first field is x.y and the second x.x.
         DNS_LINE_INV(0, { v[k] = fa; Nv[k] = fb; })
         DNS_LINE_INV(1, { u[k] = fa; Nu[k] = fa * fb; Nv[k] = fa * Nv[k] - v[k] * fb; suv += fa * v[k]; })
         DNS_LINE_INV(2, { w[k] = fa; Nw[k] = u[k] * fb; swv += fa * v[k]; })
@@ -161,7 +243,7 @@ __global__ void __launch_bounds__(SL * TPS, MINB) k_line(DnsDev d, int etlog, in
 #undef DNS_LINE_INV
 
         // forward transforms of W1 = Nu + i Nv and W2 = Nw, factorisation (R2, R1): pass A on the registers
-        group_sync<BT>();                                   // pass B of transform 5 has finished reading buf[1]
+        group_sync<GT>(grp);                                // pass B of transform 5 has finished reading buf1
         if (sl < R2) {
             double2 a1[R1], a2[R1];
 #pragma unroll
@@ -170,17 +252,17 @@ __global__ void __launch_bounds__(SL * TPS, MINB) k_line(DnsDev d, int etlog, in
             DFT<R1>::run(a2);
 #pragma unroll
             for (int k = 0; k < R1; ++k) {
-                const double2 tw = tws[sl * k];
-                buf[0][sl * PF + k * TPS + lis] = cmul(a1[k], tw);
-                buf[1][sl * PF + k * TPS + lis] = cmul(a2[k], tw);
+                const double2 tw = tws_f[k * SL + sl];
+                buf0[sl * PF + k * TPS + lis] = cmul(a1[k], tw);
+                buf1[sl * PF + k * TPS + lis] = cmul(a2[k], tw);
             }
             red[sl * TPS + lis] = make_double2(suv, swv);
         }
-        group_sync<BT>();
+        group_sync<GT>(grp);
         double2 x1[R2], x2[R2];
         if (sl < R1) {                                      // forward pass B: output n = sl + R1*k
 #pragma unroll
-            for (int i = 0; i < R2; ++i) { x1[i] = buf[0][i * PF + sl * TPS + lis]; x2[i] = buf[1][i * PF + sl * TPS + lis]; }
+            for (int i = 0; i < R2; ++i) { x1[i] = buf0[i * PF + sl * TPS + lis]; x2[i] = buf1[i * PF + sl * TPS + lis]; }
             DFT<R2>::run(x1);
             DFT<R2>::run(x2);
 #pragma unroll
@@ -191,9 +273,9 @@ __global__ void __launch_bounds__(SL * TPS, MINB) k_line(DnsDev d, int etlog, in
                 if (lo > M - NKX || pos > M - NKX) exch[(M - pos) * TPS + lis] = x1[k];
             }
         }
-        group_sync<BT>();
+        group_sync<GT>(grp);
         if (sl < R1 && lok) {
-            double2* dst = d.I3 + base;
+            double2* dst = d.I3 + ioff + lidx;
 #pragma unroll
             for (int k = 0; k < R2; ++k) {
                 const int lo = R1 * k;
@@ -202,9 +284,9 @@ __global__ void __launch_bounds__(SL * TPS, MINB) k_line(DnsDev d, int etlog, in
                 if (n < NKX) {
                     const double2 zp = x1[k], zm = n == 0 ? x1[k] : exch[n * TPS + lis];
                     // (u.grad)u = (Z(n) + conj Z(-n))/2 ; (u.grad)v = (Z(n) - conj Z(-n))/(2i) ; (u.grad)w = Z2(n)
-                    dst[(size_t)n * E] = make_double2(0.5 * (zp.x + zm.x), 0.5 * (zp.y - zm.y));
-                    dst[fstride + (size_t)n * E] = make_double2(0.5 * (zp.y + zm.y), 0.5 * (zm.x - zp.x));
-                    dst[2 * fstride + (size_t)n * E] = n == 0 ? make_double2(x2[k].x, 0.0) : x2[k];
+                    dst[n << etlog] = make_double2(0.5 * (zp.x + zm.x), 0.5 * (zp.y - zm.y));
+                    dst[fstride + (n << etlog)] = make_double2(0.5 * (zp.y + zm.y), 0.5 * (zm.x - zp.x));
+                    dst[2 * fstride + (n << etlog)] = n == 0 ? make_double2(x2[k].x, 0.0) : x2[k];
                 }
             }
             if (sl == 0) {
@@ -217,31 +299,43 @@ __global__ void __launch_bounds__(SL * TPS, MINB) k_line(DnsDev d, int etlog, in
     }
 }
 
-template <int R1, int R2, int SL, int TPS, int MINB> void line_launch(dns_plan* p) {
+template <int R1, int R2, int SL, int TPS, int NG, int NST, int MINB> void line_launch(dns_plan* p) {
     const DnsDev& d = p->d;
-    int ET = 1;
-    while (ET < TPS && ET < d.E) ET <<= 1;                  // members per group (power of two <= TPS)
-    const int etlog = __builtin_ctz(ET), LC = TPS / ET;
-    const int LQ = d.Mz % (LC * 4) == 0 ? 4 : (d.Mz % (LC * 3) == 0 ? 3 : 4);
-    const int nblk_q = (d.Mz + LC * LQ - 1) / (LC * LQ);
-    dim3 grid((unsigned)(d.Ni * nblk_q * ((d.E + ET - 1) / ET)));
-    k_line<R1, R2, SL, TPS, MINB><<<grid, SL * TPS, 0, p->stream>>>(d, etlog, LQ);
+    const LineSmem L = line_smem(R1, R2, SL, TPS, NG, NST);
+    auto kern = k_line<R1, R2, SL, TPS, NG, NST, MINB>;
+    const int LC = TPS >> d.etl;
+    const int nitems = d.Ni * ((d.Mz + LC - 1) / LC) * d.ntl;
+    if (p->line_grid == 0) {
+        cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, L.total);
+        int nb = 0, nsm = 0, dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, SL * TPS * NG, L.total);
+        if (nb < 1) nb = 1;
+        p->line_grid = nsm * nb;
+    }
+    int grid = (nitems + NG - 1) / NG;
+    if (grid > p->line_grid) grid = p->line_grid;
+    kern<<<grid, SL * TPS * NG, L.total, p->stream>>>(d, nitems);
 }
 
 }  // namespace
 
+// lanes per slot of the line kernel for padded length Mx: fixes the member tile of the mixed-array layout
+int dns_line_tps(int Mx) { return (Mx == 18 || Mx == 24 || Mx == 36 || Mx == 48) ? 4 : 8; }
+
 void launch_line(dns_plan* p) {
     switch (p->d.Mx) {
-        case 18: line_launch<3, 6, 8, 4, 16>(p); break;
-        case 24: line_launch<4, 6, 8, 4, 16>(p); break;
-        case 27: line_launch<3, 9, 12, 8, 5>(p); break;
-        case 36: line_launch<6, 6, 8, 4, 16>(p); break;
-        case 48: line_launch<6, 8, 8, 4, 16>(p); break;
-        case 54: line_launch<6, 9, 12, 8, 5>(p); break;
-        case 72: line_launch<6, 12, 12, 8, 5>(p); break;
-        case 81: line_launch<9, 9, 12, 8, 4>(p); break;
-        case 96: line_launch<8, 12, 12, 8, 3>(p); break;
-        case 108: line_launch<9, 12, 12, 8, 3>(p); break;
+        case 18: line_launch<3, 6, 8, 4, 4, 8, 3>(p); break;
+        case 24: line_launch<4, 6, 8, 4, 4, 8, 3>(p); break;
+        case 27: line_launch<3, 9, 12, 8, 1, 8, 4>(p); break;
+        case 36: line_launch<6, 6, 8, 4, 4, 8, 3>(p); break;
+        case 48: line_launch<6, 8, 8, 4, 4, 8, 3>(p); break;
+        case 54: line_launch<6, 9, 12, 8, 1, 8, 4>(p); break;
+        case 72: line_launch<6, 12, 12, 8, 1, 8, 4>(p); break;
+        case 81: line_launch<9, 9, 12, 8, 1, 4, 3>(p); break;
+        case 96: line_launch<8, 12, 12, 8, 1, 4, 3>(p); break;
+        case 108: line_launch<9, 12, 12, 8, 1, 4, 3>(p); break;
         default: break;
     }
 }
