@@ -52,9 +52,9 @@ enum {
     DNS_CLASS_FFT_Z_INV = 0, /* a4, z direction: zero-pad + i kz + complex inverse FFT            */
     DNS_CLASS_LINE = 1,      /* a4 x direction + a5 products + a6 x direction, fused per (y,z) line */
     DNS_CLASS_FFT_Z_FWD = 2, /* a6, z direction: forward FFT + truncation + 1/(Mx Mz)              */
-    DNS_CLASS_YPAIR = 3,     /* a7,a8,a9,a1,a2,a3: per-(kx,kz) DMMA contractions + stage algebra   */
-    DNS_CLASS_MEAN = 4,      /* a10: mean flow, wall lift, mass-flux gamma                          */
-    DNS_NCLASS = 5
+    DNS_CLASS_YPAIR = 3,     /* a7,a8,a9,a1,a2,a3: per-(kx,kz) DMMA contractions + stage algebra;
+                                a10 (mean flow, wall lift, mass-flux gamma) runs in the first CTAs of the same launch */
+    DNS_NCLASS = 4
 };
 
 /* dns_plan_create -- precompute everything that is constant for a fixed dt: Chebyshev D,
@@ -114,9 +114,15 @@ int dns_diagnostics(dns_plan* plan, double* out);
 /* dns_debug_fetch -- test hook: copy one INTERNAL device array to a host buffer, synchronising first.  Internal
  * spectral layout is [Ny][nkx][nkz][E] complex128 (member index fastest).  which: 0 u, 1 w, 2 du/dy, 3 dw/dy
  * (current stage, Eq. 17-18), 4 the three spectral advection terms (u.grad)u,(u.grad)v,(u.grad)w back to back,
- * 5 F^0, 6 G^0 (stage-0 nonlinear terms of Eq. 4-5, interior rows), 7 v of the current stage, 8 U00 and
+ * 5 F and 6 G history (Eq. 4-5, interior rows: F^0 after stage 0, F^0 + 4 F^1 after stage 1), 7 v of
+ * the current stage, 8 U00 and
  * 9 W00 of the current stage as [Ny][E] float64.  nbytes must equal the array size (DNS_EINVAL otherwise). */
 int dns_debug_fetch(dns_plan* plan, int which, void* host_dst, size_t nbytes);
+
+/* dns_debug_stage -- test hook: enqueue ONE Crank-Nicolson/RK3 stage (0, 1 or 2) on the
+ * plan's stream, so that per-stage internals can be fetched.  A step is stages 0, 1, 2 in order; the step
+ * counter advances after stage 2.  Errors: DNS_EINVAL (stage outside 0..2), DNS_ESTATE, DNS_ECUDA. */
+int dns_debug_stage(dns_plan* plan, int stage);
 
 /* Number of kernel launches one dns_step(1) enqueues (for bench.py's gpu_launches). */
 int dns_launches_per_step(const dns_plan* plan);

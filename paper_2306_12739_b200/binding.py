@@ -15,14 +15,15 @@ import numpy as np
 
 DNS_COUETTE, DNS_POISEUILLE_CMF = 0, 1
 DNS_OK, DNS_EINVAL, DNS_ENOMEM, DNS_ECUDA, DNS_ENONFINITE, DNS_ESTATE = 0, -1, -2, -3, -4, -5
-DNS_NCLASS = 5
-CLASS_NAMES = ("fft_z_inv", "line_fft_x_products", "fft_z_fwd", "ypair_dmma", "mean_flow")
+DNS_NCLASS = 4
+CLASS_NAMES = ("fft_z_inv", "line_fft_x_products", "fft_z_fwd", "ypair_dmma")
 
 _LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libdns_b200.so")
 _lib = None
 
 EXPORTS = ("dns_plan_create", "dns_plan_workspace_bytes", "dns_plan_bind", "dns_set_state", "dns_step",
-           "dns_step_profile", "dns_get_state", "dns_diagnostics", "dns_debug_fetch", "dns_launches_per_step", "dns_plan_destroy",
+           "dns_step_profile", "dns_get_state", "dns_diagnostics", "dns_debug_fetch", "dns_debug_stage", "dns_launches_per_step",
+           "dns_plan_destroy",
            "dns_strerror")
 
 
@@ -59,6 +60,8 @@ def lib():
         L.dns_diagnostics.restype = i
         L.dns_debug_fetch.argtypes = [vp, i, vp, ctypes.c_size_t]
         L.dns_debug_fetch.restype = i
+        L.dns_debug_stage.argtypes = [vp, i]
+        L.dns_debug_stage.restype = i
         L.dns_launches_per_step.argtypes = [vp]
         L.dns_launches_per_step.restype = i
         L.dns_plan_destroy.argtypes = [vp]
@@ -120,6 +123,10 @@ def dns_diagnostics(h, out) -> int:
 
 def dns_debug_fetch(h, which: int, out: np.ndarray) -> int:
     return lib().dns_debug_fetch(h, int(which), _ptr(out), ctypes.c_size_t(out.nbytes))
+
+
+def dns_debug_stage(h, stage: int) -> int:
+    return lib().dns_debug_stage(h, int(stage))
 
 
 def dns_launches_per_step(h) -> int:
@@ -204,6 +211,9 @@ class Plan:
         self._chk(dns_debug_fetch(self.h, which, out), "dns_debug_fetch")
         out = np.ascontiguousarray(out.transpose(0, 4, 2, 3, 1))
         return out if nf > 1 else out[0]
+
+    def debug_stage(self, stage):
+        self._chk(dns_debug_stage(self.h, stage), "dns_debug_stage")
 
     def launches_per_step(self):
         return dns_launches_per_step(self.h)

@@ -16,6 +16,12 @@ NVCC_FLAGS = [
 ]
 
 
+# The per-pair kernel is instantiated per member-tile shape; member independence must hold bit for bit across
+# instantiations (tests/test_gpu_parity.py::test_member_independence_bitwise), so the compiler may not choose
+# fused multiply-adds differently per instantiation: no contraction in that file (the DMMAs are explicit).
+EXTRA_FLAGS = {"kernels_y.cu": ["-fmad=false"]}
+
+
 def _stale() -> bool:
     if not os.path.exists(LIB):
         return True
@@ -28,13 +34,14 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not _stale():
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+    extra_env = os.environ.get("DNS_NVCC_EXTRA", "").split()          # experiments only (e.g. -DDNS_YP_REGCAP=112)
     objs = []
     procs = []
     os.makedirs(os.path.join(HERE, "build"), exist_ok=True)
     for s in SOURCES:
         o = os.path.join(HERE, "build", s.replace(".cu", ".o"))
         objs.append(o)
-        cmd = [nvcc, *NVCC_FLAGS, "-c", os.path.join(CSRC, s), "-o", o]
+        cmd = [nvcc, *NVCC_FLAGS, *EXTRA_FLAGS.get(s, []), *extra_env, "-c", os.path.join(CSRC, s), "-o", o]
         procs.append((s, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
     log = []
     for s, p in procs:

@@ -39,11 +39,11 @@ size_t carve_workspace(dns_plan* p, void* base) {
     d.vt = c.take<double2>(S);  d.et = c.take<double2>(S);  d.vs = c.take<double2>(S);
     d.uh = c.take<double2>(S);  d.wh = c.take<double2>(S);  d.duh = c.take<double2>(S);  d.dwh = c.take<double2>(S);
     d.Nh = c.take<double2>(3 * S);
-    d.F0 = c.take<double2>(S);  d.G0 = c.take<double2>(S);  d.F1 = c.take<double2>(S);  d.G1 = c.take<double2>(S);
+    d.F0 = c.take<double2>(S);  d.G0 = c.take<double2>(S);
     d.I8 = c.take<double2>(8 * I);
     d.I3 = c.take<double2>(3 * I);
     d.uvpart = c.take<double2>((size_t)d.Ny * d.Mz * d.E);
-    d.uvc0 = c.take<double2>(NE);  d.uvc1 = c.take<double2>(NE);
+    d.uvc0 = c.take<double2>(NE);
     d.Ut = c.take<double>(NE);  d.Wt = c.take<double>(NE);  d.Us = c.take<double>(NE);  d.Ws = c.take<double>(NE);
     d.gamma = c.take<double>(d.E);  d.Qstar = c.take<double>(d.E);
     d.diag = c.take<double>((size_t)d.E * 6 + NE);
@@ -64,7 +64,7 @@ bool is_device_ptr(const void* q) {
 }
 
 void run_stage(dns_plan* p, int s, cudaEvent_t* ev) {
-    // ev (optional): 6 events bracketing the 5 kernel classes
+    // ev (optional): 5 events bracketing the 4 kernel launches (the mean flow rides inside the per-pair launch)
     const double2* vin = s == 0 ? p->d.vt : p->d.vs;
     if (ev) cudaEventRecord(ev[0], p->stream);
     launch_zinv(p, vin);
@@ -75,8 +75,6 @@ void run_stage(dns_plan* p, int s, cudaEvent_t* ev) {
     if (ev) cudaEventRecord(ev[3], p->stream);
     launch_ypair(p, s, 0);
     if (ev) cudaEventRecord(ev[4], p->stream);
-    launch_mean(p, s, 0);
-    if (ev) cudaEventRecord(ev[5], p->stream);
 }
 
 }  // namespace
@@ -128,18 +126,16 @@ int dns_plan_create(dns_plan** out, int Nx, int Ny, int Nz, int E, double Re, do
     p->Lx = Lx; p->Lz = Lz;
     // member tiles
     p->ETf = pow2ceil(E) < 32 ? pow2ceil(E) : 32;
-    int ETy = pow2ceil(E) < 32 ? pow2ceil(E) : 32;
+    d.Kp = (((d.Ni + 1) / 2 + 7) / 8) * 8;
+    int ETy = pow2ceil(E) < 16 ? pow2ceil(E) : 16;
     if (ETy < 4) ETy = 4;
-    auto ysmem = [&](int et) {
-        const int NC = 2 * et, ld = (NC % 16 == 0) ? NC + 8 : NC, K = ((d.Ni + 7) / 8) * 8;
-        return (size_t)5 * K * ld * sizeof(double);
-    };
-    const size_t prefer = d.Ni <= 64 ? 110 * 1024 : 200 * 1024;
-    while (ETy > 8 && ysmem(ETy) > prefer) ETy >>= 1;
-    while (ETy > 4 && ysmem(ETy) > 220 * 1024) ETy >>= 1;
-    if (const char* s = getenv("DNS_ETY")) { int v = atoi(s); if (v == 4 || v == 8 || v == 16 || v == 32) ETy = v; }
-    if (ysmem(ETy) > 227 * 1024) { delete p; return DNS_EINVAL; }
+    while (ETy > 4 && dns_ypair_smem(d.Ni, Ny, ETy) > 75 * 1024) ETy >>= 1;
+    if (const char* s = getenv("DNS_ETY")) { int v = atoi(s); if (v == 4 || v == 8 || v == 16) ETy = v; }
+    if (dns_ypair_smem(d.Ni, Ny, ETy) > 227 * 1024) { delete p; return DNS_EINVAL; }
     p->ETy = ETy;
+    p->NTy = ETy >= 8 ? 2 : 1;
+    if (const char* s = getenv("DNS_NTY")) { int v = atoi(s); if ((v == 1 || v == 2 || v == 4) && 4 * v <= ETy) p->NTy = v; }
+    while (32 * (d.Kp / 8) * (ETy / (4 * p->NTy)) > 1024) p->NTy *= 2;
     int st = DNS_OK;
     try {
         st = dns_host_precompute(p);
@@ -188,8 +184,7 @@ int dns_set_state(dns_plan* p, const double* vhat, const double* etahat, const d
     launch_abi_to_internal(p, se, d.et);
     launch_normalise_state(p);
     launch_mean_in(p, sU, sW);
-    launch_ypair(p, 0, 1);          // derive u, w, du/dy, dw/dy of the initial state (Eq. 17-18)
-    launch_mean(p, 0, 1);
+    launch_ypair(p, 0, 1);          // derive u, w, du/dy, dw/dy of the initial state (Eq. 17-18), incl. the (0,0) column
     p->has_state = true;
     p->nsteps_done = 0;
     e = cudaGetLastError();
@@ -218,13 +213,13 @@ int dns_step_profile(dns_plan* p, int nsteps, double* ms) {
         p->ev_init = true;
     }
     for (int it = 0; it < nsteps; ++it) {
-        for (int s = 0; s < 3; ++s) run_stage(p, s, p->ev + 6 * s);
+        for (int s = 0; s < 3; ++s) run_stage(p, s, p->ev + 5 * s);
         cudaError_t e = cudaStreamSynchronize(p->stream);
         if (e != cudaSuccess) return cuda_status(p, e);
         for (int s = 0; s < 3; ++s)
             for (int c = 0; c < DNS_NCLASS; ++c) {
                 float t = 0.f;
-                cudaEventElapsedTime(&t, p->ev[6 * s + c], p->ev[6 * s + c + 1]);
+                cudaEventElapsedTime(&t, p->ev[5 * s + c], p->ev[5 * s + c + 1]);
                 ms[c] += t;
             }
         ++p->nsteps_done;
@@ -302,7 +297,16 @@ int dns_debug_fetch(dns_plan* p, int which, void* dst, size_t nbytes) {
     return cuda_status(p, e);
 }
 
-int dns_launches_per_step(const dns_plan* p) { return p ? 3 * 5 : 0; }
+int dns_debug_stage(dns_plan* p, int stage) {
+    if (!p || stage < 0 || stage > 2) return DNS_EINVAL;
+    if (p->sticky != DNS_OK) return p->sticky;
+    if (!p->bound || !p->has_state) return DNS_ESTATE;
+    run_stage(p, stage, nullptr);
+    if (stage == 2) ++p->nsteps_done;
+    return cuda_status(p, cudaGetLastError());
+}
+
+int dns_launches_per_step(const dns_plan* p) { return p ? 3 * 4 : 0; }
 
 int dns_plan_destroy(dns_plan* p) {
     if (!p) return DNS_OK;

@@ -19,8 +19,10 @@ struct DnsDev {
     const double* kz;      // [nkz] (FFT order)
     const double* w;       // [Ny] Clenshaw-Curtis weights
     const double* Dfull;   // [Ny][Ny]
-    const double* Dii;     // [Ni][Ni] interior block of D
-    const double* mats;    // [2 (h=1/2,1)][nkx*nzh][3 (Ainv, Ainv*Delinv, Sinv)][Ni*Ni]
+    // reflection-parity blocks in DMMA fragment order (plan.cu: fold_block), Kp = 8 ceil(ceil(Ni/2)/8):
+    const double* Dfrag;   // [2 (dd->s, s->dd)][Kp*Kp] interior block of D
+    const double* matsP;   // [2 (h=1/2,1)][nkx*nzh][6 (Ainv s,dd; Ainv*Delinv s,dd; Sinv s,dd)][Kp*Kp]
+    int Kp;
     const double* S0inv;   // [2][Ni*Ni]
     const double* bc;      // [2][Ni]   S0m[int,0]*U_lo + S0m[int,Ny-1]*U_hi
     const double* Ugam;    // [2][Ni]   S0inv * (h dt 1)
@@ -32,11 +34,11 @@ struct DnsDev {
     double2* vs;           // v of the current stage (transform input)
     double2 *uh, *wh, *duh, *dwh;   // u, w, du/dy, dw/dy of the current stage
     double2* Nh;           // 3 fields: (u.grad)u, (u.grad)v, (u.grad)w in spectral space
-    double2 *F0, *G0, *F1, *G1;     // stored nonlinear terms of stages 0 and 1
+    double2 *F0, *G0;      // history of the nonlinear terms: N0 after stage 0, N0 + 4 N1 after stage 1
     double2* I8;           // 8 mixed-space fields: u v w Du Dw uz vz wz
     double2* I3;           // 3 mixed-space fields: Nu Nv Nw
     double2* uvpart;       // [Ny][Mz][E] (sum_x u v, sum_x w v) per z line
-    double2 *uvc0, *uvc1;  // [Ny][E] plane means of stages 0 and 1
+    double2* uvc0;         // [Ny][E] history of the plane means (as F0, G0)
     double *Ut, *Wt, *Us, *Ws;      // mean profiles at t and at the current stage
     double *gamma, *Qstar; // [E]
     double* diag;          // [E][6] + scratch [Ny][E]
@@ -54,7 +56,7 @@ struct dns_plan {
     DnsDev d{};
     double Lx = 0, Lz = 0;
     int R1x = 0, R2x = 0, R1z = 0, R2z = 0;   // four-step factorisations of Mx, Mz
-    int ETy = 0;                               // member tile of the per-pair kernel
+    int ETy = 0, NTy = 0;                      // member tile of the per-pair kernel, n-tiles per warp
     int ETf = 0;                               // member tile of the transform kernels
     int line_grid = 0;                         // persistent grid of the line kernel (set at first launch)
     std::vector<void*> owned;                  // plan-owned device allocations
@@ -78,7 +80,7 @@ void launch_zinv(dns_plan* p, const double2* vin);
 void launch_line(dns_plan* p);
 void launch_zfwd(dns_plan* p);
 void launch_ypair(dns_plan* p, int stage, int derive_only);
-void launch_mean(dns_plan* p, int stage, int derive_only);
+size_t dns_ypair_smem(int Ni, int Ny, int ET);
 void launch_abi_to_internal(dns_plan* p, const double2* src_abi, double2* dst);
 void launch_internal_to_abi(dns_plan* p, const double2* src, double2* dst_abi);
 void launch_mean_in(dns_plan* p, const double* U_abi, const double* W_abi);

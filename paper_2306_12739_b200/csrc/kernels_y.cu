@@ -2,11 +2,17 @@
 //   k_ypair : one CTA per (kx,kz) pair and member tile.  Everything that couples only along y is chained in
 //             shared memory: F,G assembly (Eq. 4-5), RK3 combination, the precomputed-inverse
 //             solves of Eq. 12-13 for ALL members of the tile at once, dv/dy, the u,w
-//             reconstruction of Eq. 17-18 and du/dy, dw/dy.  The contractions are [Ni x Ni] x [Ni x 2 ET] fp64
-//             tensor-core MMAs (DMMA.8x8x4; the only fp64 MMA shape sm_100a executes natively).
-//   k_mean  : mean profiles U00, W00 (Eq. 14-15) with the wall lift f+-  and the mass-flux
-//             pressure gamma solved so that the discrete bulk flux is held.
+//             reconstruction of Eq. 17-18 and du/dy, dw/dy.  The contractions run on the fp64 tensor cores
+//             (DMMA.8x8x4; the only fp64 MMA shape sm_100a executes natively) in the REFLECTION-PARITY basis:
+//             with J the reversal y -> -y of the interior Gauss-Lobatto points, the Chebyshev matrix obeys
+//             J D J = -D and every solve matrix J M J = M, so in the variables s = x + Jx, dd = x - Jx each
+//             [Ni x Ni] product splits into two [Ni/2 x Ni/2] ones: half the flops and half the matrix bytes.
+//             The first CTAs of the grid do the mean flow instead (row a10): U00, W00 of Eq. 14-15 with the wall
+//             lift f+-  and the mass-flux pressure gamma solved so that the discrete bulk flux is
+//             held; they run in the shadow of the pair CTAs.
 // plus layout conversion, input normalisation and diagnostics.
+#include <cstdint>
+
 #include "dns_internal.h"
 
 namespace {
@@ -17,20 +23,52 @@ __device__ __forceinline__ void dmma(double (&c)[2], double a, double b) {
                  : "d"(a), "d"(b));
 }
 
-// acc[nt] += A[rows 8w..8w+7][0..Ni) * Bs[0..K)[8nt..8nt+7];  A row-major in global memory (ld = Ni), Bs in
-// shared memory with leading dimension ld (rows >= Ni are zero).
-template <int NT>
-__device__ __forceinline__ void gemm_acc(double (&acc)[NT][2], const double* __restrict__ A, const double* Bs,
-                                         int Ni, int K, int ld, int r, int t, int g) {
-    const bool rok = r < Ni;
-    const double* Ar = A + (size_t)(rok ? r : 0) * Ni;
-#pragma unroll 4
-    for (int k0 = 0; k0 < K; k0 += 4) {
-        const int k = k0 + t;
-        const double a = (rok && k < Ni) ? __ldg(Ar + k) : 0.0;
-        const double* bp = Bs + (size_t)k * ld + g;
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred P1;\n"
+        "LAB_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+        "@P1 bra DONE;\n"
+        "bra LAB_WAIT;\n"
+        "DONE:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+
+// acc[nt] += Ablk[rows 8 mt .. 8 mt + 7][0..8 KS2) * B[.][col0 + 8 nt ..+7].  Ablk is one parity block in DMMA
+// fragment order (plan.cu: fold_block): a warp reads 512 contiguous bytes per pair of k-steps.  B is a parity
+// panel in shared memory: row k of the s part is smem row k, row k of the dd part is smem row Ni-1-k (REV).
+template <int NT, int KS2T, bool REV>
+__device__ __forceinline__ void gemm_blk(double (&acc)[NT][2], const double* __restrict__ Ablk, const double* Bp,
+                                         int KS2r, int mt, int lane, int ld, int Ni, int col0) {
+    const int KS2 = KS2T ? KS2T : KS2r;
+    const int g = lane >> 2, t = lane & 3;
+    const double2* Af = reinterpret_cast<const double2*>(Ablk) + (size_t)mt * KS2 * 32 + lane;
+    const double* Bc = Bp + col0 + g;
 #pragma unroll
-        for (int nt = 0; nt < NT; ++nt) dmma(acc[nt], a, bp[8 * nt]);
+    for (int ks2 = 0; ks2 < KS2; ++ks2) {
+        const double2 a2 = __ldg(Af + ks2 * 32);
+        const int k = 8 * ks2 + t;
+        const int r0 = REV ? max(Ni - 1 - k, 0) : min(k, Ni - 1);
+        const int r1 = REV ? max(Ni - 5 - k, 0) : min(k + 4, Ni - 1);
+        const double* b0 = Bc + r0 * ld;
+        const double* b1 = Bc + r1 * ld;
+#pragma unroll
+        for (int nt = 0; nt < NT; ++nt) dmma(acc[nt], a2.x, b0[8 * nt]);
+#pragma unroll
+        for (int nt = 0; nt < NT; ++nt) dmma(acc[nt], a2.y, b1[8 * nt]);
     }
 }
 
@@ -39,154 +77,14 @@ template <int NT> __device__ __forceinline__ void zero_acc(double (&acc)[NT][2])
     for (int nt = 0; nt < NT; ++nt) acc[nt][0] = acc[nt][1] = 0.0;
 }
 
-// grid = (P-1) * ntile_e ; block = 32 * MT, MT = ceil(Ni/8); dynamic smem = 5 panels of K x ld doubles
-template <int NT>
-__global__ void k_ypair(DnsDev d, int stage, int derive_only) {
-    extern __shared__ double smy[];
-    constexpr int NC = 8 * NT, ET = 4 * NT;
-    constexpr int ld = (NC % 16 == 0) ? NC + 8 : NC;    // row stride = 64 B mod 128 B: conflict-free B fragments
-    const int Ni = d.Ni, MT = blockDim.x >> 5, K = MT * 8;
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
-    const int ntile_e = (d.E + ET - 1) / ET;
-    const int p = 1 + blockIdx.x / ntile_e, e0 = (blockIdx.x % ntile_e) * ET;
-    const int n = p / d.nkz, mi = p % d.nkz;
-    const int mabs = mi < d.nzh ? mi : d.nkz - mi;
-    const double kx = d.kx[n], kz = d.kz[mi], alpha = kx * kx + kz * kz;
-    const int hi = stage == 0 ? 0 : 1;
-    const double hdt = (stage == 0 ? 0.5 : 1.0) * d.dt;
-    const size_t NN = (size_t)Ni * Ni;
-    const double* mAinv = d.mats + (((size_t)hi * d.nkx * d.nzh + (size_t)n * d.nzh + mabs) * 3) * NN;
-    const double* mAD = mAinv + NN;
-    const double* mSinv = mAD + NN;
-    const size_t PS = (size_t)K * ld;
-    double* P0 = smy;
-    double* P1 = P0 + PS;
-    double* P2 = P1 + PS;
-    double* P3 = P2 + PS;
-    double* P4 = P3 + PS;
-    const int r = 8 * warp + g;                         // interior row owned in every fragment
-    const bool rok = r < Ni;
-    // global offset of element (row r, pair p, member e0 + 4nt + t)
-    const size_t gbase = ((size_t)(r + 1) * d.P + p) * d.E + e0 + t;
-    auto eok = [&](int nt) { return rok && (e0 + 4 * nt + t) < d.E; };
-    auto sidx = [&](int nt) { return (size_t)r * ld + 8 * nt + 2 * t; };
-    const double2 Z2 = make_double2(0.0, 0.0);
-    double2* vout = stage == 2 ? d.vt : d.vs;
-
-    // zero every panel once (padding rows >= Ni and padding columns must hold finite zeros)
-    for (size_t i = threadIdx.x; i < 5 * PS; i += blockDim.x) smy[i] = 0.0;
-    __syncthreads();
-
-    double acc[NT][2];
-    if (!derive_only) {
-        // ---- A: H = i kx Nu + i kz Nw -> P0 ; G = i kz Nu - i kx Nw, RK3 combination, eta rhs -> P1
-#pragma unroll
-        for (int nt = 0; nt < NT; ++nt) {
-            if (!eok(nt)) continue;
-            const size_t gi = gbase + 4 * nt;
-            const double2 nu = d.Nh[gi], nw = d.Nh[2 * d.S + gi];
-            const double2 H = make_double2(-kx * nu.y - kz * nw.y, kx * nu.x + kz * nw.x);
-            double2 G = make_double2(-kz * nu.y + kx * nw.y, kz * nu.x - kx * nw.x);      // Eq. 5
-            double2 Gc;
-            if (stage == 0) { d.G0[gi] = G; Gc = G; }
-            else if (stage == 1) { const double2 g0 = d.G0[gi]; d.G1[gi] = G; Gc = make_double2(2.0 * G.x - g0.x, 2.0 * G.y - g0.y); }
-            else { const double2 g0 = d.G0[gi], g1 = d.G1[gi];
-                   Gc = make_double2((g0.x + 4.0 * g1.x + G.x) / 6.0, (g0.y + 4.0 * g1.y + G.y) / 6.0); }
-            const double2 et = d.et[gi];
-            P0[sidx(nt)] = H.x; P0[sidx(nt) + 1] = H.y;
-            P1[sidx(nt)] = 2.0 * et.x - hdt * Gc.x; P1[sidx(nt) + 1] = 2.0 * et.y - hdt * Gc.y;
-        }
-        __syncthreads();
-        // ---- B: F = -alpha Nv - D H (Eq. 4 with Eq. 10's sign), RK3 combination; -h dt Fc -> P2 ; 2 v_t -> P3
-        zero_acc<NT>(acc);
-        gemm_acc<NT>(acc, d.Dii, P0, Ni, K, ld, r, t, g);
-#pragma unroll
-        for (int nt = 0; nt < NT; ++nt) {
-            if (!eok(nt)) continue;
-            const size_t gi = gbase + 4 * nt;
-            const double2 nv = d.Nh[d.S + gi];
-            const double2 F = make_double2(-alpha * nv.x - acc[nt][0], -alpha * nv.y - acc[nt][1]);
-            double2 Fc;
-            if (stage == 0) { d.F0[gi] = F; Fc = F; }
-            else if (stage == 1) { const double2 f0 = d.F0[gi]; d.F1[gi] = F; Fc = make_double2(2.0 * F.x - f0.x, 2.0 * F.y - f0.y); }
-            else { const double2 f0 = d.F0[gi], f1 = d.F1[gi];
-                   Fc = make_double2((f0.x + 4.0 * f1.x + F.x) / 6.0, (f0.y + 4.0 * f1.y + F.y) / 6.0); }
-            const double2 vt = d.vt[gi];
-            P2[sidx(nt)] = -hdt * Fc.x; P2[sidx(nt) + 1] = -hdt * Fc.y;
-            P3[sidx(nt)] = 2.0 * vt.x;  P3[sidx(nt) + 1] = 2.0 * vt.y;
-        }
-        __syncthreads();
-        // ---- C: v' = Ainv (2 v_t) + AD (-h dt Fc) - v_t (Eq. 12) -> global, P0 ; eta' = Sinv P1 - eta_t (Eq. 13) -> P4
-        zero_acc<NT>(acc);
-        gemm_acc<NT>(acc, mAinv, P3, Ni, K, ld, r, t, g);
-        gemm_acc<NT>(acc, mAD, P2, Ni, K, ld, r, t, g);
-        double acc2[NT][2];
-        zero_acc<NT>(acc2);
-        gemm_acc<NT>(acc2, mSinv, P1, Ni, K, ld, r, t, g);
-        __syncthreads();                                 // every warp has finished reading P0..P3
-#pragma unroll
-        for (int nt = 0; nt < NT; ++nt) {
-            if (!eok(nt)) continue;
-            const size_t gi = gbase + 4 * nt;
-            const double2 vn = make_double2(acc[nt][0] - 0.5 * P3[sidx(nt)], acc[nt][1] - 0.5 * P3[sidx(nt) + 1]);
-            const double2 et = d.et[gi];
-            const double2 en = make_double2(acc2[nt][0] - et.x, acc2[nt][1] - et.y);
-            vout[gi] = vn;
-            if (stage == 2) d.et[gi] = en;
-            P0[sidx(nt)] = vn.x; P0[sidx(nt) + 1] = vn.y;
-            P4[sidx(nt)] = en.x; P4[sidx(nt) + 1] = en.y;
-        }
-        __syncthreads();
-    } else {
-#pragma unroll
-        for (int nt = 0; nt < NT; ++nt) {
-            if (!eok(nt)) continue;
-            const size_t gi = gbase + 4 * nt;
-            const double2 vt = d.vt[gi], et = d.et[gi];
-            P0[sidx(nt)] = vt.x; P0[sidx(nt) + 1] = vt.y;
-            P4[sidx(nt)] = et.x; P4[sidx(nt) + 1] = et.y;
-        }
-        __syncthreads();
-    }
-    // ---- D: dv/dy = D v' ; u = (i kx Dv - i kz eta)/alpha, w = (i kz Dv + i kx eta)/alpha (Eq. 17-18) -> global, P2, P3
-    zero_acc<NT>(acc);
-    gemm_acc<NT>(acc, d.Dii, P0, Ni, K, ld, r, t, g);
-#pragma unroll
-    for (int nt = 0; nt < NT; ++nt) {
-        if (!eok(nt)) continue;
-        const size_t gi = gbase + 4 * nt;
-        const double2 dv = make_double2(acc[nt][0], acc[nt][1]);
-        const double2 en = make_double2(P4[sidx(nt)], P4[sidx(nt) + 1]);
-        const double2 u = make_double2((-kx * dv.y + kz * en.y) / alpha, (kx * dv.x - kz * en.x) / alpha);
-        const double2 w = make_double2((-kz * dv.y - kx * en.y) / alpha, (kz * dv.x + kx * en.x) / alpha);
-        d.uh[gi] = u;
-        d.wh[gi] = w;
-        P2[sidx(nt)] = u.x; P2[sidx(nt) + 1] = u.y;
-        P3[sidx(nt)] = w.x; P3[sidx(nt) + 1] = w.y;
-    }
-    __syncthreads();
-    // ---- E: du/dy, dw/dy
-    zero_acc<NT>(acc);
-    gemm_acc<NT>(acc, d.Dii, P2, Ni, K, ld, r, t, g);
-    double acc2[NT][2];
-    zero_acc<NT>(acc2);
-    gemm_acc<NT>(acc2, d.Dii, P3, Ni, K, ld, r, t, g);
-#pragma unroll
-    for (int nt = 0; nt < NT; ++nt) {
-        if (!eok(nt)) continue;
-        const size_t gi = gbase + 4 * nt;
-        d.duh[gi] = make_double2(acc[nt][0], acc[nt][1]);
-        d.dwh[gi] = make_double2(acc2[nt][0], acc2[nt][1]);
-    }
-    (void)Z2;
-}
+__device__ __forceinline__ double2 ld2(const double* p) { return *reinterpret_cast<const double2*>(p); }
+__device__ __forceinline__ void st2(double* p, double2 v) { *reinterpret_cast<double2*>(p) = v; }
 
 // ------------------------------------------------------------------------------------------------ mean flow
-// grid = ceil(E/8); block = 256 = 32 row slots x 8 members; dynamic smem = 6 vectors [Ny][8]
-__global__ void __launch_bounds__(256) k_mean(DnsDev d, int stage, int derive_only) {
-    extern __shared__ double smm[];
-    const int Ny = d.Ny, Ni = d.Ni;
-    const int el = threadIdx.x & 7, rs = threadIdx.x >> 3, e = blockIdx.x * 8 + el;
+// CTA-wide: tiles of 8 members x (blockDim/8) row slots; dynamic smem = 6 vectors [Ny][8]
+__device__ void mean_body(const DnsDev& d, int stage, int derive_only, int tile, double* smm) {
+    const int Ny = d.Ny, Ni = d.Ni, nrs = blockDim.x >> 3;
+    const int el = threadIdx.x & 7, rs = threadIdx.x >> 3, e = tile * 8 + el;
     const bool eok = e < d.E;
     const int hi = stage == 0 ? 0 : 1;
     const double hdt = (stage == 0 ? 0.5 : 1.0) * d.dt;
@@ -201,7 +99,7 @@ __global__ void __launch_bounds__(256) k_mean(DnsDev d, int stage, int derive_on
     double* Wout = stage == 2 ? d.Wt : d.Ws;
     if (!derive_only) {
         // plane means [uv]00, [wv]00 (Eq. 6-7): fixed-order sum of the per-line partial sums
-        for (int j = rs; j < Ny; j += 32) {
+        for (int j = rs; j < Ny; j += nrs) {
             double a = 0.0, b = 0.0;
             if (eok && j > 0 && j < Ny - 1) {
                 for (int q = 0; q < d.Mz; ++q) {
@@ -209,16 +107,17 @@ __global__ void __launch_bounds__(256) k_mean(DnsDev d, int stage, int derive_on
                     a += v.x; b += v.y;
                 }
                 a *= d.invMxMz; b *= d.invMxMz;
+                // history: stage 0 stores S0, stage 1 replaces it by S0 + 4 S1
                 const size_t gi = (size_t)j * d.E + e;
                 if (stage == 0) d.uvc0[gi] = make_double2(a, b);
-                else if (stage == 1) { const double2 s0 = d.uvc0[gi]; d.uvc1[gi] = make_double2(a, b); a = 2.0 * a - s0.x; b = 2.0 * b - s0.y; }
-                else { const double2 s0 = d.uvc0[gi], s1 = d.uvc1[gi]; a = (s0.x + 4.0 * s1.x + a) / 6.0; b = (s0.y + 4.0 * s1.y + b) / 6.0; }
+                else if (stage == 1) { const double2 s0 = d.uvc0[gi]; d.uvc0[gi] = make_double2(s0.x + 4.0 * a, s0.y + 4.0 * b); a = 2.0 * a - s0.x; b = 2.0 * b - s0.y; }
+                else { const double2 s01 = d.uvc0[gi]; a = (s01.x + a) / 6.0; b = (s01.y + b) / 6.0; }
             }
             uvc[j * 8 + el] = a; wvc[j * 8 + el] = b;
         }
         __syncthreads();
         // rhs = 2 U_t - h dt D [uv] - 2 bc  (Eq. 14 with S0p = 2I - S0m and the wall columns on the rhs)
-        for (int i = rs; i < Ni; i += 32) {
+        for (int i = rs; i < Ni; i += nrs) {
             double su = 0.0, sw = 0.0;
             const double* Dr = d.Dfull + (size_t)(i + 1) * Ny;
             for (int j = 1; j < Ny - 1; ++j) { su += Dr[j] * uvc[j * 8 + el]; sw += Dr[j] * wvc[j * 8 + el]; }
@@ -227,7 +126,7 @@ __global__ void __launch_bounds__(256) k_mean(DnsDev d, int stage, int derive_on
             rw[i * 8 + el] = 2.0 * wt - hdt * sw;
         }
         __syncthreads();
-        for (int i = rs; i < Ni; i += 32) {
+        for (int i = rs; i < Ni; i += nrs) {
             double su = 0.0, sw = 0.0;
             const double* Sr = d.S0inv + (size_t)hi * Ni * Ni + (size_t)i * Ni;
             for (int k = 0; k < Ni; ++k) { su += Sr[k] * ru[k * 8 + el]; sw += Sr[k] * rw[k * 8 + el]; }
@@ -248,7 +147,7 @@ __global__ void __launch_bounds__(256) k_mean(DnsDev d, int stage, int derive_on
             if (eok) d.gamma[e] = gm;
         }
         __syncthreads();
-        for (int j = rs; j < Ny; j += 32) {
+        for (int j = rs; j < Ny; j += nrs) {
             double un = Un[j * 8 + el];
             if (j > 0 && j < Ny - 1) un += gam[el] * d.Ugam[hi * Ni + j - 1];
             Un[j * 8 + el] = un;
@@ -256,14 +155,14 @@ __global__ void __launch_bounds__(256) k_mean(DnsDev d, int stage, int derive_on
         }
         __syncthreads();
     } else {
-        for (int j = rs; j < Ny; j += 32) {
+        for (int j = rs; j < Ny; j += nrs) {
             Un[j * 8 + el] = eok ? d.Ut[(size_t)j * d.E + e] : 0.0;
             Wn[j * 8 + el] = eok ? d.Wt[(size_t)j * d.E + e] : 0.0;
         }
         __syncthreads();
     }
     // (0,0) column of the transform inputs: u = U00, w = W00, du/dy = D U00, dw/dy = D W00
-    for (int j = rs; j < Ny; j += 32) {
+    for (int j = rs; j < Ny; j += nrs) {
         double du = 0.0, dw = 0.0;
         const double* Dr = d.Dfull + (size_t)j * Ny;
         for (int k = 0; k < Ny; ++k) { du += Dr[k] * Un[k * 8 + el]; dw += Dr[k] * Wn[k * 8 + el]; }
@@ -273,6 +172,301 @@ __global__ void __launch_bounds__(256) k_mean(DnsDev d, int stage, int derive_on
             d.wh[gi] = make_double2(Wn[j * 8 + el], 0.0);
             d.duh[gi] = make_double2(du, 0.0);
             d.dwh[gi] = make_double2(dw, 0.0);
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ per-pair chain
+// grid = nmean + (P-1) * ntile_e ; block = 32 * (Kp/8) * NWN ; dynamic smem = 5 panels of Ni x ld doubles.
+// A warp owns m-tile mt (rows 8 mt..+7 of BOTH parities) and NT n-tiles (members 4 NT wn .. of the tile).
+#ifndef DNS_YP_REGCAP
+#define DNS_YP_REGCAP 128
+#endif
+// CTAs per SM the register allocation is asked to allow: as many as fit with DNS_YP_REGCAP registers per thread
+constexpr int ypair_minb(int threads) {
+    return threads == 0 ? 1 : (65536 / (threads * DNS_YP_REGCAP) > 0 ? 65536 / (threads * DNS_YP_REGCAP) : 1);
+}
+
+template <int NT, int NWNT, int KS2T>
+__global__ void __launch_bounds__(KS2T ? 32 * KS2T * NWNT : 1024, ypair_minb(32 * KS2T * NWNT))
+k_ypair(DnsDev d, int stage, int derive_only, int nmean) {
+    extern __shared__ __align__(128) double smy[];
+    __shared__ uint64_t bar;
+    if ((int)blockIdx.x < nmean) { mean_body(d, stage, derive_only, blockIdx.x, smy); return; }
+    const int bid = blockIdx.x - nmean;
+    const int Ni = d.Ni, KS2 = KS2T ? KS2T : (d.Kp >> 3), Kp = 8 * KS2, Kh = (Ni + 1) >> 1, Kho = Ni >> 1;
+    constexpr int NWN = NWNT, NC = 8 * NT * NWN, ET = NC >> 1, ld = NC + 4;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
+    const int mt = warp % KS2, wn = warp / KS2;
+    const int ntile_e = (d.E + ET - 1) / ET;
+    const int p = 1 + bid / ntile_e, e0 = (bid % ntile_e) * ET;
+    const int n = p / d.nkz, mi = p % d.nkz;
+    const int mabs = mi < d.nzh ? mi : d.nkz - mi;
+    const double kx = d.kx[n], kz = d.kz[mi], alpha = kx * kx + kz * kz, ialpha = 1.0 / alpha;
+    const int hi = stage == 0 ? 0 : 1;
+    const double hdt = (stage == 0 ? 0.5 : 1.0) * d.dt;
+    const size_t BB = (size_t)Kp * Kp;
+    const double* mA = d.matsP + (((size_t)hi * d.nkx * d.nzh + (size_t)n * d.nzh + mabs) * 6) * BB;
+    const double* Dsd = d.Dfrag;            // dd -> s
+    const double* Dds = d.Dfrag + BB;       // s -> dd
+    const size_t PS = (size_t)Ni * ld;
+    double* P0 = smy;
+    double* P1 = P0 + PS;
+    double* P2 = P1 + PS;
+    double* P3 = P2 + PS;
+    double* P4 = P3 + PS;
+    const size_t rowstride = (size_t)d.P * d.E;             // complex elements between consecutive y rows
+    const size_t pbase = (size_t)p * d.E + e0;              // + (row + 1) * rowstride + member
+    double2* vout = stage == 2 ? d.vt : d.vs;
+
+    // ---- stage the inputs: one bulk copy per (field, row) into the padded panel rows, all in flight at once
+    const int nvalid = d.E - e0 < ET ? d.E - e0 : ET;
+    const uint32_t rowbytes = (uint32_t)nvalid * 16u;
+    const int nf = derive_only ? 2 : 5;
+    if (threadIdx.x == 0) {
+        mbar_init(&bar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) mbar_arrive_expect_tx(&bar, (uint32_t)(nf * Ni) * rowbytes);
+    for (int it = threadIdx.x; it < nf * Ni; it += blockDim.x) {
+        const int f = it / Ni, r = it - f * Ni;
+        const double2* src;
+        double* dst;
+        if (derive_only) { src = f == 0 ? d.vt : d.et; dst = f == 0 ? P0 : P4; }
+        else {
+            src = f == 0 ? d.Nh : f == 1 ? d.Nh + 2 * d.S : f == 2 ? d.Nh + d.S : f == 3 ? d.vt : d.et;
+            dst = smy + (size_t)f * PS;
+        }
+        bulk_g2s(dst + (size_t)r * ld, src + pbase + (size_t)(r + 1) * rowstride, rowbytes, &bar);
+    }
+
+    // ---- own fragment elements: row i = 8 mt + g of both parities, columns col0 + 8 nt + 2t, +1 (one member)
+    const int i = 8 * mt + g, Ji = Ni - 1 - i;
+    const bool sok = i < Kh, dok = i < Kho;
+    const int col0 = 8 * NT * wn;
+    const int offS = (sok ? i : 0) * ld + col0 + 2 * t, offD = (dok ? Ji : 0) * ld + col0 + 2 * t;
+    auto eokf = [&](int nt) { return (e0 + (col0 >> 1) + 4 * nt + t) < d.E; };
+    const size_t gS = pbase + (size_t)(i + 1) * rowstride + (col0 >> 1) + t;      // + 4 nt : natural row i
+    const size_t gD = pbase + (size_t)(Ji + 1) * rowstride + (col0 >> 1) + t;     // natural row J i
+
+    // ---- history of the nonlinear terms: hist = N0 after stage 0, N0 + 4 N1 after stage 1
+    double2 fhS[NT], fhD[NT], ghA[NT], ghB[NT];
+    if (!derive_only && stage > 0) {
+#pragma unroll
+        for (int nt = 0; nt < NT; ++nt) {
+            fhS[nt] = fhD[nt] = make_double2(0.0, 0.0);
+            if (eokf(nt)) {
+                if (sok) fhS[nt] = d.F0[gS + 4 * nt];
+                if (dok) fhD[nt] = d.F0[gD + 4 * nt];
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < NT; ++k) {
+            const int q = threadIdx.x + k * blockDim.x, ia = q / ET, e = q - ia * ET;
+            ghA[k] = ghB[k] = make_double2(0.0, 0.0);
+            if (ia < Kh && e < nvalid) {
+                ghA[k] = d.G0[pbase + (size_t)(ia + 1) * rowstride + e];
+                ghB[k] = d.G0[pbase + (size_t)(Ni - ia) * rowstride + e];
+            }
+        }
+    }
+    mbar_wait(&bar, 0);
+
+    double accS[NT][2], accD[NT][2];
+    if (!derive_only) {
+        // ---- A (element-wise, in place): natural rows (ia, J ia) -> parity rows; H = i kx Nu + i kz Nw -> P0,
+        //      G = i kz Nu - i kx Nw (Eq. 5), RK3 combination, 2 eta_t - h dt Gc -> P1, Nv -> P2, 2 v_t -> P3, eta_t -> P4
+#pragma unroll
+        for (int k = 0; k < NT; ++k) {
+            const int q = threadIdx.x + k * blockDim.x, ia = q / ET, e = q - ia * ET;
+            if (ia >= Kh) continue;
+            const int ib = Ni - 1 - ia;
+            double* a0 = P0 + ia * ld + 2 * e;
+            double* b0 = P0 + ib * ld + 2 * e;
+            const double2 nuA = ld2(a0), nuB = ld2(b0), nwA = ld2(a0 + PS), nwB = ld2(b0 + PS);
+            const double2 nvA = ld2(a0 + 2 * PS), nvB = ld2(b0 + 2 * PS), vtA = ld2(a0 + 3 * PS), vtB = ld2(b0 + 3 * PS);
+            const double2 etA = ld2(a0 + 4 * PS), etB = ld2(b0 + 4 * PS);
+            const double2 HA = make_double2(-kx * nuA.y - kz * nwA.y, kx * nuA.x + kz * nwA.x);
+            const double2 HB = make_double2(-kx * nuB.y - kz * nwB.y, kx * nuB.x + kz * nwB.x);
+            const double2 GA = make_double2(-kz * nuA.y + kx * nwA.y, kz * nuA.x - kx * nwA.x);
+            const double2 GB = make_double2(-kz * nuB.y + kx * nwB.y, kz * nuB.x - kx * nwB.x);
+            double2 GcA, GcB;
+            const bool eok = e < nvalid;
+            const size_t giA = pbase + (size_t)(ia + 1) * rowstride + e, giB = pbase + (size_t)(ib + 1) * rowstride + e;
+            if (stage == 0) {
+                GcA = GA; GcB = GB;
+                if (eok) { d.G0[giA] = GA; d.G0[giB] = GB; }
+            } else if (stage == 1) {
+                GcA = make_double2(2.0 * GA.x - ghA[k].x, 2.0 * GA.y - ghA[k].y);
+                GcB = make_double2(2.0 * GB.x - ghB[k].x, 2.0 * GB.y - ghB[k].y);
+                if (eok) {
+                    d.G0[giA] = make_double2(ghA[k].x + 4.0 * GA.x, ghA[k].y + 4.0 * GA.y);
+                    d.G0[giB] = make_double2(ghB[k].x + 4.0 * GB.x, ghB[k].y + 4.0 * GB.y);
+                }
+            } else {
+                GcA = make_double2((ghA[k].x + GA.x) / 6.0, (ghA[k].y + GA.y) / 6.0);
+                GcB = make_double2((ghB[k].x + GB.x) / 6.0, (ghB[k].y + GB.y) / 6.0);
+            }
+            const double2 rA = make_double2(2.0 * etA.x - hdt * GcA.x, 2.0 * etA.y - hdt * GcA.y);
+            const double2 rB = make_double2(2.0 * etB.x - hdt * GcB.x, 2.0 * etB.y - hdt * GcB.y);
+            st2(a0, make_double2(HA.x + HB.x, HA.y + HB.y));
+            st2(a0 + PS, make_double2(rA.x + rB.x, rA.y + rB.y));
+            st2(a0 + 2 * PS, make_double2(nvA.x + nvB.x, nvA.y + nvB.y));
+            st2(a0 + 3 * PS, make_double2(2.0 * (vtA.x + vtB.x), 2.0 * (vtA.y + vtB.y)));
+            st2(a0 + 4 * PS, make_double2(etA.x + etB.x, etA.y + etB.y));
+            if (ib != ia) {
+                st2(b0, make_double2(HA.x - HB.x, HA.y - HB.y));
+                st2(b0 + PS, make_double2(rA.x - rB.x, rA.y - rB.y));
+                st2(b0 + 2 * PS, make_double2(nvA.x - nvB.x, nvA.y - nvB.y));
+                st2(b0 + 3 * PS, make_double2(2.0 * (vtA.x - vtB.x), 2.0 * (vtA.y - vtB.y)));
+                st2(b0 + 4 * PS, make_double2(etA.x - etB.x, etA.y - etB.y));
+            }
+        }
+        __syncthreads();
+        // ---- B: F = -alpha Nv - D H (Eq. 4 with Eq. 10's sign), RK3 combination; -h dt Fc -> P2
+        zero_acc<NT>(accS); zero_acc<NT>(accD);
+        gemm_blk<NT, KS2T, true>(accS, Dsd, P0, KS2, mt, lane, ld, Ni, col0);
+        gemm_blk<NT, KS2T, false>(accD, Dds, P0, KS2, mt, lane, ld, Ni, col0);
+#pragma unroll
+        for (int nt = 0; nt < NT; ++nt) {
+            double2 FS = make_double2(0.0, 0.0), FD = make_double2(0.0, 0.0);
+            if (sok) { const double2 nv = ld2(P2 + offS + 8 * nt); FS = make_double2(-alpha * nv.x - accS[nt][0], -alpha * nv.y - accS[nt][1]); }
+            if (dok) { const double2 nv = ld2(P2 + offD + 8 * nt); FD = make_double2(-alpha * nv.x - accD[nt][0], -alpha * nv.y - accD[nt][1]); }
+            // natural rows: F(i) = (FS + FD)/2, F(Ji) = (FS - FD)/2
+            const double2 FA = make_double2(0.5 * (FS.x + FD.x), 0.5 * (FS.y + FD.y));
+            const double2 FB = make_double2(0.5 * (FS.x - FD.x), 0.5 * (FS.y - FD.y));
+            double2 cA, cB;
+            const bool eok = eokf(nt);
+            if (stage == 0) {
+                cA = FA; cB = FB;
+                if (eok && sok) d.F0[gS + 4 * nt] = FA;
+                if (eok && dok) d.F0[gD + 4 * nt] = FB;
+            } else if (stage == 1) {
+                cA = make_double2(2.0 * FA.x - fhS[nt].x, 2.0 * FA.y - fhS[nt].y);
+                cB = make_double2(2.0 * FB.x - fhD[nt].x, 2.0 * FB.y - fhD[nt].y);
+                if (eok && sok) d.F0[gS + 4 * nt] = make_double2(fhS[nt].x + 4.0 * FA.x, fhS[nt].y + 4.0 * FA.y);
+                if (eok && dok) d.F0[gD + 4 * nt] = make_double2(fhD[nt].x + 4.0 * FB.x, fhD[nt].y + 4.0 * FB.y);
+            } else {
+                cA = make_double2((fhS[nt].x + FA.x) / 6.0, (fhS[nt].y + FA.y) / 6.0);
+                cB = make_double2((fhD[nt].x + FB.x) / 6.0, (fhD[nt].y + FB.y) / 6.0);
+            }
+            if (!dok) cB = cA;                              // middle row of an odd Ni: s = 2 x
+            if (sok) st2(P2 + offS + 8 * nt, make_double2(-hdt * (cA.x + cB.x), -hdt * (cA.y + cB.y)));
+            if (dok) st2(P2 + offD + 8 * nt, make_double2(-hdt * (cA.x - cB.x), -hdt * (cA.y - cB.y)));
+        }
+        __syncthreads();
+        // ---- C: v' = Ainv (2 v_t) + AD (-h dt Fc) - v_t (Eq. 12) -> global, P0 ; eta' = Sinv P1 - eta_t (Eq. 13) -> P4
+        zero_acc<NT>(accS); zero_acc<NT>(accD);
+        gemm_blk<NT, KS2T, false>(accS, mA, P3, KS2, mt, lane, ld, Ni, col0);
+        gemm_blk<NT, KS2T, true>(accD, mA + BB, P3, KS2, mt, lane, ld, Ni, col0);
+        gemm_blk<NT, KS2T, false>(accS, mA + 2 * BB, P2, KS2, mt, lane, ld, Ni, col0);
+        gemm_blk<NT, KS2T, true>(accD, mA + 3 * BB, P2, KS2, mt, lane, ld, Ni, col0);
+        double acc2S[NT][2], acc2D[NT][2];
+        zero_acc<NT>(acc2S); zero_acc<NT>(acc2D);
+        gemm_blk<NT, KS2T, false>(acc2S, mA + 4 * BB, P1, KS2, mt, lane, ld, Ni, col0);
+        gemm_blk<NT, KS2T, true>(acc2D, mA + 5 * BB, P1, KS2, mt, lane, ld, Ni, col0);
+#pragma unroll
+        for (int nt = 0; nt < NT; ++nt) {
+            double2 vS = make_double2(0.0, 0.0), vD = vS, eS = vS, eD = vS;
+            if (sok) {
+                const double2 v2 = ld2(P3 + offS + 8 * nt), et = ld2(P4 + offS + 8 * nt);
+                vS = make_double2(accS[nt][0] - 0.5 * v2.x, accS[nt][1] - 0.5 * v2.y);
+                eS = make_double2(acc2S[nt][0] - et.x, acc2S[nt][1] - et.y);
+                st2(P0 + offS + 8 * nt, vS);
+                st2(P4 + offS + 8 * nt, eS);
+            }
+            if (dok) {
+                const double2 v2 = ld2(P3 + offD + 8 * nt), et = ld2(P4 + offD + 8 * nt);
+                vD = make_double2(accD[nt][0] - 0.5 * v2.x, accD[nt][1] - 0.5 * v2.y);
+                eD = make_double2(acc2D[nt][0] - et.x, acc2D[nt][1] - et.y);
+                st2(P0 + offD + 8 * nt, vD);
+                st2(P4 + offD + 8 * nt, eD);
+            }
+            if (eokf(nt)) {
+                if (sok) {
+                    vout[gS + 4 * nt] = make_double2(0.5 * (vS.x + vD.x), 0.5 * (vS.y + vD.y));
+                    if (stage == 2) d.et[gS + 4 * nt] = make_double2(0.5 * (eS.x + eD.x), 0.5 * (eS.y + eD.y));
+                }
+                if (dok) {
+                    vout[gD + 4 * nt] = make_double2(0.5 * (vS.x - vD.x), 0.5 * (vS.y - vD.y));
+                    if (stage == 2) d.et[gD + 4 * nt] = make_double2(0.5 * (eS.x - eD.x), 0.5 * (eS.y - eD.y));
+                }
+            }
+        }
+        __syncthreads();
+    } else {
+        // parity transform of v_t (P0) and eta_t (P4) in place
+#pragma unroll
+        for (int k = 0; k < NT; ++k) {
+            const int q = threadIdx.x + k * blockDim.x, ia = q / ET, e = q - ia * ET;
+            if (ia >= Kh) continue;
+            const int ib = Ni - 1 - ia;
+            double* a0 = P0 + ia * ld + 2 * e;
+            double* b0 = P0 + ib * ld + 2 * e;
+            const double2 vA = ld2(a0), vB = ld2(b0), eA = ld2(a0 + 4 * PS), eB = ld2(b0 + 4 * PS);
+            st2(a0, make_double2(vA.x + vB.x, vA.y + vB.y));
+            st2(a0 + 4 * PS, make_double2(eA.x + eB.x, eA.y + eB.y));
+            if (ib != ia) {
+                st2(b0, make_double2(vA.x - vB.x, vA.y - vB.y));
+                st2(b0 + 4 * PS, make_double2(eA.x - eB.x, eA.y - eB.y));
+            }
+        }
+        __syncthreads();
+    }
+    // ---- D: dv/dy = D v' ; u = (i kx Dv - i kz eta)/alpha, w = (i kz Dv + i kx eta)/alpha (Eq. 17-18) -> global, P2, P3
+    zero_acc<NT>(accS); zero_acc<NT>(accD);
+    gemm_blk<NT, KS2T, true>(accS, Dsd, P0, KS2, mt, lane, ld, Ni, col0);
+    gemm_blk<NT, KS2T, false>(accD, Dds, P0, KS2, mt, lane, ld, Ni, col0);
+#pragma unroll
+    for (int nt = 0; nt < NT; ++nt) {
+        double2 uS = make_double2(0.0, 0.0), uD = uS, wS = uS, wD = uS;
+        if (sok) {
+            const double2 en = ld2(P4 + offS + 8 * nt);
+            uS = make_double2((-kx * accS[nt][1] + kz * en.y) * ialpha, (kx * accS[nt][0] - kz * en.x) * ialpha);
+            wS = make_double2((-kz * accS[nt][1] - kx * en.y) * ialpha, (kz * accS[nt][0] + kx * en.x) * ialpha);
+            st2(P2 + offS + 8 * nt, uS);
+            st2(P3 + offS + 8 * nt, wS);
+        }
+        if (dok) {
+            const double2 en = ld2(P4 + offD + 8 * nt);
+            uD = make_double2((-kx * accD[nt][1] + kz * en.y) * ialpha, (kx * accD[nt][0] - kz * en.x) * ialpha);
+            wD = make_double2((-kz * accD[nt][1] - kx * en.y) * ialpha, (kz * accD[nt][0] + kx * en.x) * ialpha);
+            st2(P2 + offD + 8 * nt, uD);
+            st2(P3 + offD + 8 * nt, wD);
+        }
+        if (eokf(nt)) {
+            if (sok) {
+                d.uh[gS + 4 * nt] = make_double2(0.5 * (uS.x + uD.x), 0.5 * (uS.y + uD.y));
+                d.wh[gS + 4 * nt] = make_double2(0.5 * (wS.x + wD.x), 0.5 * (wS.y + wD.y));
+            }
+            if (dok) {
+                d.uh[gD + 4 * nt] = make_double2(0.5 * (uS.x - uD.x), 0.5 * (uS.y - uD.y));
+                d.wh[gD + 4 * nt] = make_double2(0.5 * (wS.x - wD.x), 0.5 * (wS.y - wD.y));
+            }
+        }
+    }
+    __syncthreads();
+    // ---- E: du/dy, dw/dy
+    {
+        double a2S[NT][2], a2D[NT][2];
+        zero_acc<NT>(accS); zero_acc<NT>(accD); zero_acc<NT>(a2S); zero_acc<NT>(a2D);
+        gemm_blk<NT, KS2T, true>(accS, Dsd, P2, KS2, mt, lane, ld, Ni, col0);
+        gemm_blk<NT, KS2T, false>(accD, Dds, P2, KS2, mt, lane, ld, Ni, col0);
+        gemm_blk<NT, KS2T, true>(a2S, Dsd, P3, KS2, mt, lane, ld, Ni, col0);
+        gemm_blk<NT, KS2T, false>(a2D, Dds, P3, KS2, mt, lane, ld, Ni, col0);
+#pragma unroll
+        for (int nt = 0; nt < NT; ++nt) {
+            if (!eokf(nt)) continue;
+            if (sok) {
+                d.duh[gS + 4 * nt] = make_double2(0.5 * (accS[nt][0] + accD[nt][0]), 0.5 * (accS[nt][1] + accD[nt][1]));
+                d.dwh[gS + 4 * nt] = make_double2(0.5 * (a2S[nt][0] + a2D[nt][0]), 0.5 * (a2S[nt][1] + a2D[nt][1]));
+            }
+            if (dok) {
+                d.duh[gD + 4 * nt] = make_double2(0.5 * (accS[nt][0] - accD[nt][0]), 0.5 * (accS[nt][1] - accD[nt][1]));
+                d.dwh[gD + 4 * nt] = make_double2(0.5 * (a2S[nt][0] - a2D[nt][0]), 0.5 * (a2S[nt][1] - a2D[nt][1]));
+            }
         }
     }
 }
@@ -381,35 +575,41 @@ __global__ void k_diag_rows(DnsDev d, const double* __restrict__ part, double t)
 
 }  // namespace
 
-static size_t ypair_smem(int Ni, int NT) {
-    const int NC = 8 * NT, ld = (NC % 16 == 0) ? NC + 8 : NC, K = ((Ni + 7) / 8) * 8;
-    return (size_t)5 * K * ld * sizeof(double);
+size_t dns_ypair_smem(int Ni, int Ny, int ET) {
+    const size_t panels = (size_t)5 * Ni * (2 * ET + 4) * sizeof(double), mean = (size_t)6 * Ny * 8 * sizeof(double);
+    return panels > mean ? panels : mean;
 }
 
-void launch_ypair(dns_plan* p, int stage, int derive_only) {
+template <int NT, int NWN> static void ypair_launch(dns_plan* p, int stage, int derive_only) {
     const DnsDev& d = p->d;
-    const int MT = (d.Ni + 7) / 8, ET = p->ETy, NT = ET / 4;
-    const unsigned grid = (unsigned)((d.P - 1) * ((d.E + ET - 1) / ET));
-    const size_t smem = ypair_smem(d.Ni, NT);
-#define LAUNCH(NTv)                                                                                   \
+    const int KS2 = d.Kp >> 3, ET = 4 * NT * NWN;
+    const int nmean = (d.E + 7) / 8;
+    const unsigned grid = (unsigned)(nmean + (d.P - 1) * ((d.E + ET - 1) / ET));
+    const size_t smem = dns_ypair_smem(d.Ni, d.Ny, ET);
+#define LAUNCH(K)                                                                                     \
     {                                                                                                 \
-        auto kern = k_ypair<NTv>;                                                                     \
+        auto kern = k_ypair<NT, NWN, K>;                                                              \
         cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);           \
-        kern<<<grid, 32 * MT, smem, p->stream>>>(d, stage, derive_only);                              \
+        kern<<<grid, 32 * KS2 * NWN, smem, p->stream>>>(d, stage, derive_only, nmean);                \
     }
-    switch (NT) {
-        case 1: LAUNCH(1) break;
+    switch (KS2) {
         case 2: LAUNCH(2) break;
+        case 3: LAUNCH(3) break;
         case 4: LAUNCH(4) break;
-        default: LAUNCH(8) break;
+        case 6: LAUNCH(6) break;
+        default: LAUNCH(0) break;
     }
 #undef LAUNCH
 }
 
-void launch_mean(dns_plan* p, int stage, int derive_only) {
-    const DnsDev& d = p->d;
-    const size_t smem = (size_t)6 * d.Ny * 8 * sizeof(double);
-    k_mean<<<(d.E + 7) / 8, 256, smem, p->stream>>>(d, stage, derive_only);
+void launch_ypair(dns_plan* p, int stage, int derive_only) {
+    const int NT = p->NTy, NWN = p->ETy / (4 * NT);
+    if (NT == 1 && NWN == 1) ypair_launch<1, 1>(p, stage, derive_only);
+    else if (NT == 2 && NWN == 1) ypair_launch<2, 1>(p, stage, derive_only);
+    else if (NT == 1 && NWN == 2) ypair_launch<1, 2>(p, stage, derive_only);
+    else if (NT == 2 && NWN == 2) ypair_launch<2, 2>(p, stage, derive_only);
+    else if (NT == 4 && NWN == 1) ypair_launch<4, 1>(p, stage, derive_only);
+    else ypair_launch<1, 4>(p, stage, derive_only);
 }
 
 void launch_abi_to_internal(dns_plan* p, const double2* src, double2* dst) {

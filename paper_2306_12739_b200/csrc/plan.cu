@@ -10,6 +10,14 @@
 //   v'   = Ainv (2 v_t) + AD (-h dt F) - v_t          (Eq. 12)
 //   eta' = Sinv (2 eta_t - h dt G) - eta_t            (Eq. 13)
 // i.e. three matrices per pair instead of the paper's four (ICg, ICgCg and their v counterparts).
+//
+// Reflection parity.  With J the reversal of the interior Gauss-Lobatto points (y -> -y), D is centro-antisymmetric
+// (J D J = -D) and Ainv, AD, Sinv are centrosymmetric (J M J = M).  In the variables s = x + Jx, dd = x - Jx (first
+// half of the rows; the middle row of an odd Ni carries s = 2x, dd = 0) a product y = M x becomes
+//   ys = Ms s,  yd = Md dd,   Ms(i,j) = M(i,j) + M(i,Jj),  Md(i,j) = M(i,j) - M(i,Jj)      (centrosymmetric)
+//   ys = Dsd dd, yd = Dds s,  Dsd(i,j) = D(i,j) - D(i,Jj), Dds(i,j) = D(i,j) + D(i,Jj)     (centro-antisymmetric)
+// (the middle column is not doubled).  Only these half-size blocks are stored, in the order the DMMA.8x8x4 A
+// fragments consume them, so the per-pair kernel does half the flops on half the matrix bytes.
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -95,6 +103,21 @@ static bool invert(const Mat& A, Mat& Ainv, int n) {
     for (int i = 0; i < n; ++i) Ainv[(size_t)i * n + i] = 1.0L;
     lu_solve(LU, piv, Ainv, n);
     return true;
+}
+
+// Kp x Kp parity block of the Ni x Ni matrix M in DMMA fragment order: element (i, j) of m-tile i/8 and k-step
+// pair j/8 sits at (((i/8) (Kp/8) + j/8) 32 + 4 (i%8) + j%4) 2 + (j/4)%2.  sign = +1: columns j < ceil(Ni/2);
+// sign = -1: columns j < floor(Ni/2).  Rows >= nrows and unused columns stay zero.
+static void fold_block(const Mat& M, int Ni, int Kp, int sign, int nrows, double* out) {
+    const int ncols = sign > 0 ? (Ni + 1) / 2 : Ni / 2, KS2 = Kp / 8;
+    for (int i = 0; i < nrows; ++i)
+        for (int j = 0; j < ncols; ++j) {
+            const int Jj = Ni - 1 - j;
+            real v = M[(size_t)i * Ni + j];
+            if (Jj != j) v += sign * M[(size_t)i * Ni + Jj];
+            const size_t idx = ((((size_t)(i >> 3) * KS2 + (j >> 3)) * 32 + 4 * (i & 7) + (j & 3)) << 1) + ((j >> 2) & 1);
+            out[idx] = (double)v;
+        }
 }
 
 bool dns_factor_len(int M, int* R1, int* R2) {
@@ -198,7 +221,9 @@ int dns_host_precompute(dns_plan* p) {
     // ---- per-(alpha, h) inverses (Listing 1 + Listing 3, Eq. 12-13)
     const int nA = d.nkx * d.nzh;
     const size_t NN = (size_t)Ni * Ni;
-    std::vector<double> mats((size_t)2 * nA * 3 * NN, 0.0);
+    const int Kp = d.Kp, Kh = (Ni + 1) / 2, Kho = Ni / 2;
+    const size_t BB = (size_t)Kp * Kp;
+    std::vector<double> mats((size_t)2 * nA * 6 * BB, 0.0);
     int fail = 0;
     const real dt = d.dt, Re = d.Re;
 #pragma omp parallel for schedule(dynamic, 1)
@@ -231,12 +256,13 @@ int dns_host_precompute(dns_plan* p) {
             for (int i = 0; i < Ni; ++i) { A[(size_t)i * Ni + i] += 1.0L; Sm[(size_t)i * Ni + i] += 1.0L; }
             if (!invert(A, Ainv, Ni) || !invert(Sm, Sinv, Ni)) { fail = 1; continue; }
             matmul(Ainv, Delinv, AD, Ni);
-            double* out = &mats[(((size_t)hi * nA + a) * 3) * NN];
-            for (size_t i = 0; i < NN; ++i) {
-                out[i] = (double)Ainv[i];
-                out[NN + i] = (double)AD[i];
-                out[2 * NN + i] = (double)Sinv[i];
-            }
+            double* out = &mats[(((size_t)hi * nA + a) * 6) * BB];
+            fold_block(Ainv, Ni, Kp, +1, Kh, out);
+            fold_block(Ainv, Ni, Kp, -1, Kho, out + BB);
+            fold_block(AD, Ni, Kp, +1, Kh, out + 2 * BB);
+            fold_block(AD, Ni, Kp, -1, Kho, out + 3 * BB);
+            fold_block(Sinv, Ni, Kp, +1, Kh, out + 4 * BB);
+            fold_block(Sinv, Ni, Kp, -1, Kho, out + 5 * BB);
         }
     }
     if (fail) return DNS_EINVAL;
@@ -265,16 +291,17 @@ int dns_host_precompute(dns_plan* p) {
         d.wUg[hi] = (double)(0.5L * wug);
     }
     // ---- upload
-    std::vector<double> Dfull_d((size_t)Ny * Ny), Dii_d(NN);
+    std::vector<double> Dfull_d((size_t)Ny * Ny), Dfrag_d(2 * BB, 0.0);
     for (size_t i = 0; i < Dfull_d.size(); ++i) Dfull_d[i] = (double)D[i];
-    for (size_t i = 0; i < NN; ++i) Dii_d[i] = (double)Dii[i];
+    fold_block(Dii, Ni, Kp, -1, Kh, Dfrag_d.data());          // dd -> s
+    fold_block(Dii, Ni, Kp, +1, Kho, Dfrag_d.data() + BB);    // s -> dd
     cudaError_t err = cudaSuccess;
     d.kx = upload(p, kx, &err);
     d.kz = upload(p, kz, &err);
     d.w = upload(p, w, &err);
     d.Dfull = upload(p, Dfull_d, &err);
-    d.Dii = upload(p, Dii_d, &err);
-    d.mats = upload(p, mats, &err);
+    d.Dfrag = upload(p, Dfrag_d, &err);
+    d.matsP = upload(p, mats, &err);
     d.S0inv = upload(p, S0inv, &err);
     d.bc = upload(p, bc, &err);
     d.Ugam = upload(p, Ugam, &err);

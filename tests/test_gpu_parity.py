@@ -267,7 +267,7 @@ def test_stage_pieces_against_oracle():
         got = plan.debug_fetch(which)
         assert field_err(got[..., 1:-1], ref[..., 1:-1]) < 1e-12, which
     F, G, Su, Sw = o.nonlinear(o.v, o.eta, o.U, o.W)
-    plan.step(1)
+    plan.debug_stage(0)                       # after stage 0 the history buffers hold F^0, G^0
     assert field_err(plan.debug_fetch(5)[..., 1:-1], F) < 1e-11
     assert field_err(plan.debug_fetch(6)[..., 1:-1], G) < 1e-11
     plan.close()
