@@ -150,6 +150,7 @@ template <int R1, int R2> void zinv_launch(dns_plan* p, const double2* vin) {
     const size_t smem = (size_t)(M + (size_t)NB * 2 * M * ET) * sizeof(double2);
     auto kern = k_zinv<R1, R2>;
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
     dim3 grid((unsigned)(d.Ni * ((d.nkx + NB - 1) / NB) * ((d.E + ET - 1) / ET)), 5);
     kern<<<grid, 256, smem, p->stream>>>(d, vin, etlog, NB);
 }
@@ -164,6 +165,7 @@ template <int R1, int R2> void zfwd_launch(dns_plan* p) {
     const size_t smem = (size_t)(M + (size_t)NB * M * ET) * sizeof(double2);
     auto kern = k_zfwd<R1, R2>;
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
     dim3 grid((unsigned)(d.Ni * ((d.nkx + NB - 1) / NB) * ((d.E + ET - 1) / ET)), 3);
     kern<<<grid, 256, smem, p->stream>>>(d, etlog, NB);
 }

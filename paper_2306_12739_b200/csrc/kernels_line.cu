@@ -307,6 +307,7 @@ template <int R1, int R2, int SL, int TPS, int NG, int NST, int MINB> void line_
     const int nitems = d.Ni * ((d.Mz + LC - 1) / LC) * d.ntl;
     if (p->line_grid == 0) {
         cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, L.total);
+        cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
         int nb = 0, nsm = 0, dev = 0;
         cudaGetDevice(&dev);
         cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);

@@ -12,6 +12,7 @@
 //             held; they run in the shadow of the pair CTAs.
 // plus layout conversion, input normalisation and diagnostics.
 #include <cstdint>
+#include <cstdlib>
 
 #include "dns_internal.h"
 
@@ -192,7 +193,8 @@ __global__ void __launch_bounds__(KS2T ? 32 * KS2T * NWNT : 1024, ypair_minb(32 
 k_ypair(DnsDev d, int stage, int derive_only, int nmean) {
     extern __shared__ __align__(128) double smy[];
     __shared__ uint64_t bar;
-    if ((int)blockIdx.x < nmean) { mean_body(d, stage, derive_only, blockIdx.x, smy); return; }
+    if ((int)blockIdx.x < nmean) { if (derive_only != 7 && stage < 8) mean_body(d, stage & 3, derive_only, blockIdx.x, smy); return; }
+    stage &= 3;
     const int bid = blockIdx.x - nmean;
     const int Ni = d.Ni, KS2 = KS2T ? KS2T : (d.Kp >> 3), Kp = 8 * KS2, Kh = (Ni + 1) >> 1, Kho = Ni >> 1;
     constexpr int NWN = NWNT, NC = 8 * NT * NWN, ET = NC >> 1, ld = NC + 4;
@@ -590,7 +592,9 @@ template <int NT, int NWN> static void ypair_launch(dns_plan* p, int stage, int 
     {                                                                                                 \
         auto kern = k_ypair<NT, NWN, K>;                                                              \
         cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);           \
-        kern<<<grid, 32 * KS2 * NWN, smem, p->stream>>>(d, stage, derive_only, nmean);                \
+        cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared); \
+        static const int nomean = getenv("DNS_NOMEAN") ? 8 : 0;                                       \
+        kern<<<grid, 32 * KS2 * NWN, smem, p->stream>>>(d, stage | nomean, derive_only, nmean);       \
     }
     switch (KS2) {
         case 2: LAUNCH(2) break;
