@@ -47,6 +47,7 @@ size_t carve_workspace(dns_plan* p, void* base) {
     d.Ut = c.take<double>(NE);  d.Wt = c.take<double>(NE);  d.Us = c.take<double>(NE);  d.Ws = c.take<double>(NE);
     d.gamma = c.take<double>(d.E);  d.Qstar = c.take<double>(d.E);
     d.diag = c.take<double>((size_t)d.E * 6 + NE);
+    d.ypctr = c.take<unsigned int>(64);
     d.stage_io = c.take<double2>(2 * S + 2 * NE);
     return c.off;
 }
@@ -129,7 +130,7 @@ int dns_plan_create(dns_plan** out, int Nx, int Ny, int Nz, int E, double Re, do
     d.Kp = (((d.Ni + 1) / 2 + 7) / 8) * 8;
     int ETy = pow2ceil(E) < 16 ? pow2ceil(E) : 16;
     if (ETy < 4) ETy = 4;
-    while (ETy > 4 && dns_ypair_smem(d.Ni, Ny, ETy) > 75 * 1024) ETy >>= 1;
+    while (ETy > 4 && dns_ypair_smem(d.Ni, Ny, ETy) > 76 * 1024) ETy >>= 1;
     if (const char* s = getenv("DNS_ETY")) { int v = atoi(s); if (v == 4 || v == 8 || v == 16) ETy = v; }
     if (dns_ypair_smem(d.Ni, Ny, ETy) > 227 * 1024) { delete p; return DNS_EINVAL; }
     p->ETy = ETy;
@@ -158,6 +159,8 @@ int dns_plan_bind(dns_plan* p, void* ws, size_t bytes, void* stream) {
     p->workspace = ws;
     p->stream = static_cast<cudaStream_t>(stream);
     carve_workspace(p, ws);
+    const int st = dns_ypair_encode_maps(p);
+    if (st != DNS_OK) { p->sticky = st; return st; }
     p->bound = true;
     p->has_state = false;
     return cuda_status(p, cudaMemsetAsync(ws, 0, p->workspace_bytes, p->stream));

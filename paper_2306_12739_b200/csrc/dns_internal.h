@@ -42,6 +42,7 @@ struct DnsDev {
     double *Ut, *Wt, *Us, *Ws;      // mean profiles at t and at the current stage
     double *gamma, *Qstar; // [E]
     double* diag;          // [E][6] + scratch [Ny][E]
+    unsigned int* ypctr;   // [2] work counter / exit counter of the persistent per-pair kernel (zero between launches)
     double2* stage_io;     // staging for ABI-layout copies: 2 spectral fields
     size_t S;              // Ny*P*E
     size_t Isz;            // Ny*Mz*ntl*nkx*2^etl
@@ -59,6 +60,8 @@ struct dns_plan {
     int ETy = 0, NTy = 0;                      // member tile of the per-pair kernel, n-tiles per warp
     int ETf = 0;                               // member tile of the transform kernels
     int line_grid = 0;                         // persistent grid of the line kernel (set at first launch)
+    int ypair_grid = 0;                        // persistent grid of the per-pair kernel (set at first launch)
+    alignas(64) unsigned char tmaps[3][128];   // CUtensorMap of Nh, vt, et (encoded at dns_plan_bind)
     std::vector<void*> owned;                  // plan-owned device allocations
     void* workspace = nullptr;
     size_t workspace_bytes = 0;
@@ -81,6 +84,7 @@ void launch_line(dns_plan* p);
 void launch_zfwd(dns_plan* p);
 void launch_ypair(dns_plan* p, int stage, int derive_only);
 size_t dns_ypair_smem(int Ni, int Ny, int ET);
+int dns_ypair_encode_maps(dns_plan* p);
 void launch_abi_to_internal(dns_plan* p, const double2* src_abi, double2* dst);
 void launch_internal_to_abi(dns_plan* p, const double2* src, double2* dst_abi);
 void launch_mean_in(dns_plan* p, const double* U_abi, const double* W_abi);

@@ -1,16 +1,22 @@
 // Wall-normal part of one stage (north_star subsystems (3), (4)).
-//   k_ypair : one CTA per (kx,kz) pair and member tile.  Everything that couples only along y is chained in
-//             shared memory: F,G assembly (Eq. 4-5), RK3 combination, the precomputed-inverse
-//             solves of Eq. 12-13 for ALL members of the tile at once, dv/dy, the u,w
-//             reconstruction of Eq. 17-18 and du/dy, dw/dy.  The contractions run on the fp64 tensor cores
-//             (DMMA.8x8x4; the only fp64 MMA shape sm_100a executes natively) in the REFLECTION-PARITY basis:
-//             with J the reversal y -> -y of the interior Gauss-Lobatto points, the Chebyshev matrix obeys
-//             J D J = -D and every solve matrix J M J = M, so in the variables s = x + Jx, dd = x - Jx each
-//             [Ni x Ni] product splits into two [Ni/2 x Ni/2] ones: half the flops and half the matrix bytes.
-//             The first CTAs of the grid do the mean flow instead (row a10): U00, W00 of Eq. 14-15 with the wall
-//             lift f+-  and the mass-flux pressure gamma solved so that the discrete bulk flux is
-//             held; they run in the shadow of the pair CTAs.
+//   k_ypair : persistent CTAs walk over work items (one (kx,kz) pair, one member tile).  Everything that couples
+//             only along y is chained in shared memory: F,G assembly (Eq. 4-5), RK3 combination,
+//             the precomputed-inverse solves of Eq. 12-13 for ALL members of the tile at once,
+//             dv/dy, the u,w reconstruction of Eq. 17-18 and du/dy, dw/dy.  The contractions run on the fp64
+//             tensor cores (DMMA.8x8x4; the only fp64 MMA shape sm_100a executes natively) in the
+//             REFLECTION-PARITY basis: with J the reversal y -> -y of the interior Gauss-Lobatto points, the
+//             Chebyshev matrix obeys J D J = -D and every solve matrix J M J = M, so in the variables
+//             s = x + Jx, dd = x - Jx each [Ni x Ni] product splits into two [Ni/2 x Ni/2] ones: half the
+//             flops and half the matrix bytes.
+//             Inputs arrive by TMA (one cp.async.bulk.tensor per field and item: box = Ni rows x one member
+//             tile, landing directly in the padded panel layout) into a second panel set while the previous
+//             item is being computed, so HBM streams under the DMMA chain.  Items are handed out by an atomic
+//             counter; the CTAs with the lowest indices first do the mean flow (row a10): U00, W00 of
+//             Eq. 14-15 with the wall lift f+-  and the mass-flux pressure gamma solved so that
+//             the discrete bulk flux is held.
 // plus layout conversion, input normalisation and diagnostics.
+#include <cuda.h>
+
 #include <cstdint>
 #include <cstdlib>
 
@@ -42,34 +48,42 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
         "DONE:\n"
         "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
 }
-__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
-                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
+// one 2-D tile (box fixed by the tensor map: ld doubles x Ni rows) -> shared memory, completion on an mbarrier
+__device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* tm, int c0, int c1, uint64_t* bar) {
+    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(
+                     smem_u32(dst)),
+                 "l"(tm), "r"(c0), "r"(c1), "r"(smem_u32(bar))
                  : "memory");
 }
 
-// acc[nt] += Ablk[rows 8 mt .. 8 mt + 7][0..8 KS2) * B[.][col0 + 8 nt ..+7].  Ablk is one parity block in DMMA
-// fragment order (plan.cu: fold_block): a warp reads 512 contiguous bytes per pair of k-steps.  B is a parity
-// panel in shared memory: row k of the s part is smem row k, row k of the dd part is smem row Ni-1-k (REV).
-template <int NT, int KS2T, bool REV>
-__device__ __forceinline__ void gemm_blk(double (&acc)[NT][2], const double* __restrict__ Ablk, const double* Bp,
-                                         int KS2r, int mt, int lane, int ld, int Ni, int col0) {
+// One k-sweep of two parity blocks at once (four independent accumulator chains per n-tile pair keep the DMMA
+// pipe busy):  accS[nt] += AS[rows 8 mt..+7][:] * B_S[:][col0 + 8 nt..+7],  accD likewise with AD, B_D.
+// AS, AD are parity blocks in DMMA fragment order (plan.cu: fold_block): a warp reads 512 contiguous bytes per
+// pair of k-steps.  The B operands are parity panels in shared memory: row k of the s part is smem row k, row k
+// of the dd part is smem row Ni-1-k (REV).
+template <int NT, int KS2T, bool REVS, bool REVD>
+__device__ __forceinline__ void gemm2(double (&accS)[NT][2], double (&accD)[NT][2], const double* __restrict__ AS,
+                                      const double* __restrict__ AD, const double* BS, const double* BD, int KS2r,
+                                      int mt, int lane, int ld, int Ni, int col0) {
     const int KS2 = KS2T ? KS2T : KS2r;
     const int g = lane >> 2, t = lane & 3;
-    const double2* Af = reinterpret_cast<const double2*>(Ablk) + (size_t)mt * KS2 * 32 + lane;
-    const double* Bc = Bp + col0 + g;
+    const double2* AfS = reinterpret_cast<const double2*>(AS) + (size_t)mt * KS2 * 32 + lane;
+    const double2* AfD = reinterpret_cast<const double2*>(AD) + (size_t)mt * KS2 * 32 + lane;
+    const double* BcS = BS + col0 + g;
+    const double* BcD = BD + col0 + g;
 #pragma unroll
     for (int ks2 = 0; ks2 < KS2; ++ks2) {
-        const double2 a2 = __ldg(Af + ks2 * 32);
+        const double2 aS = __ldg(AfS + ks2 * 32), aD = __ldg(AfD + ks2 * 32);
         const int k = 8 * ks2 + t;
-        const int r0 = REV ? max(Ni - 1 - k, 0) : min(k, Ni - 1);
-        const int r1 = REV ? max(Ni - 5 - k, 0) : min(k + 4, Ni - 1);
-        const double* b0 = Bc + r0 * ld;
-        const double* b1 = Bc + r1 * ld;
+        const int f0 = min(k, Ni - 1), f1 = min(k + 4, Ni - 1), r0 = max(Ni - 1 - k, 0), r1 = max(Ni - 5 - k, 0);
+        const double* s0 = BcS + (REVS ? r0 : f0) * ld;
+        const double* s1 = BcS + (REVS ? r1 : f1) * ld;
+        const double* d0 = BcD + (REVD ? r0 : f0) * ld;
+        const double* d1 = BcD + (REVD ? r1 : f1) * ld;
 #pragma unroll
-        for (int nt = 0; nt < NT; ++nt) dmma(acc[nt], a2.x, b0[8 * nt]);
+        for (int nt = 0; nt < NT; ++nt) { dmma(accS[nt], aS.x, s0[8 * nt]); dmma(accD[nt], aD.x, d0[8 * nt]); }
 #pragma unroll
-        for (int nt = 0; nt < NT; ++nt) dmma(acc[nt], a2.y, b1[8 * nt]);
+        for (int nt = 0; nt < NT; ++nt) { dmma(accS[nt], aS.y, s1[8 * nt]); dmma(accD[nt], aD.y, d1[8 * nt]); }
     }
 }
 
@@ -178,298 +192,319 @@ __device__ void mean_body(const DnsDev& d, int stage, int derive_only, int tile,
 }
 
 // ------------------------------------------------------------------------------------------------ per-pair chain
-// grid = nmean + (P-1) * ntile_e ; block = 32 * (Kp/8) * NWN ; dynamic smem = 5 panels of Ni x ld doubles.
-// A warp owns m-tile mt (rows 8 mt..+7 of BOTH parities) and NT n-tiles (members 4 NT wn .. of the tile).
 #ifndef DNS_YP_REGCAP
-#define DNS_YP_REGCAP 128
+#define DNS_YP_REGCAP 112
 #endif
 // CTAs per SM the register allocation is asked to allow: as many as fit with DNS_YP_REGCAP registers per thread
 constexpr int ypair_minb(int threads) {
     return threads == 0 ? 1 : (65536 / (threads * DNS_YP_REGCAP) > 0 ? 65536 / (threads * DNS_YP_REGCAP) : 1);
 }
 
+// grid = persistent CTAs ; block = 32 * (Kp/8) * NWN ; dynamic smem = 2 sets of 5 panels of Ni x ld doubles.
+// A warp owns m-tile mt (rows 8 mt..+7 of BOTH parities) and NT n-tiles (members 4 NT wn .. of the tile).
+// Work item it = (pair p = 1 + it / ntile_e, member tile it % ntile_e), handed out by d.ypctr[0].
 template <int NT, int NWNT, int KS2T>
 __global__ void __launch_bounds__(KS2T ? 32 * KS2T * NWNT : 1024, ypair_minb(32 * KS2T * NWNT))
-k_ypair(DnsDev d, int stage, int derive_only, int nmean) {
+k_ypair(DnsDev d, const __grid_constant__ CUtensorMap tmN, const __grid_constant__ CUtensorMap tmV,
+        const __grid_constant__ CUtensorMap tmE, int stage, int derive_only, int nmean, int nitems) {
     extern __shared__ __align__(128) double smy[];
-    __shared__ uint64_t bar;
-    if ((int)blockIdx.x < nmean) { if (derive_only != 7 && stage < 8) mean_body(d, stage & 3, derive_only, blockIdx.x, smy); return; }
-    stage &= 3;
-    const int bid = blockIdx.x - nmean;
+    __shared__ uint64_t bar[2];
+    __shared__ int s_item[2];
+    if ((int)blockIdx.x < nmean) mean_body(d, stage, derive_only, blockIdx.x, smy);
     const int Ni = d.Ni, KS2 = KS2T ? KS2T : (d.Kp >> 3), Kp = 8 * KS2, Kh = (Ni + 1) >> 1, Kho = Ni >> 1;
     constexpr int NWN = NWNT, NC = 8 * NT * NWN, ET = NC >> 1, ld = NC + 4;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
     const int mt = warp % KS2, wn = warp / KS2;
     const int ntile_e = (d.E + ET - 1) / ET;
-    const int p = 1 + bid / ntile_e, e0 = (bid % ntile_e) * ET;
-    const int n = p / d.nkz, mi = p % d.nkz;
-    const int mabs = mi < d.nzh ? mi : d.nkz - mi;
-    const double kx = d.kx[n], kz = d.kz[mi], alpha = kx * kx + kz * kz, ialpha = 1.0 / alpha;
     const int hi = stage == 0 ? 0 : 1;
     const double hdt = (stage == 0 ? 0.5 : 1.0) * d.dt;
     const size_t BB = (size_t)Kp * Kp;
-    const double* mA = d.matsP + (((size_t)hi * d.nkx * d.nzh + (size_t)n * d.nzh + mabs) * 6) * BB;
     const double* Dsd = d.Dfrag;            // dd -> s
     const double* Dds = d.Dfrag + BB;       // s -> dd
-    const size_t PS = (size_t)Ni * ld;
-    double* P0 = smy;
-    double* P1 = P0 + PS;
-    double* P2 = P1 + PS;
-    double* P3 = P2 + PS;
-    double* P4 = P3 + PS;
-    const size_t rowstride = (size_t)d.P * d.E;             // complex elements between consecutive y rows
-    const size_t pbase = (size_t)p * d.E + e0;              // + (row + 1) * rowstride + member
+    const size_t PS = ((size_t)Ni * ld + 15) & ~(size_t)15;      // panel pitch: a multiple of 128 B (TMA destination)
+    const size_t rowstride = (size_t)d.P * d.E;                  // complex elements between consecutive y rows
     double2* vout = stage == 2 ? d.vt : d.vs;
-
-    // ---- stage the inputs: one bulk copy per (field, row) into the padded panel rows, all in flight at once
-    const int nvalid = d.E - e0 < ET ? d.E - e0 : ET;
-    const uint32_t rowbytes = (uint32_t)nvalid * 16u;
     const int nf = derive_only ? 2 : 5;
+    const uint32_t txbytes = (uint32_t)(nf * Ni * ld * 8);
+
+    // thread 0: fetch the inputs of item `it` into panel set b (box = Ni rows x ld doubles; the 4 pad columns
+    // of every row are the first two members of the neighbouring tile: never used)
+    auto issue = [&](int it, int b) {
+        const int p = 1 + it / ntile_e, e0 = (it % ntile_e) * ET;
+        const int c0 = 2 * (p * d.E + e0);
+        double* base = smy + (size_t)b * 5 * PS;
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");      // panel set b was last written by st.shared
+        mbar_arrive_expect_tx(&bar[b], txbytes);
+        if (derive_only) {
+            tma_load_2d(base, &tmV, c0, 1, &bar[b]);
+            tma_load_2d(base + 4 * PS, &tmE, c0, 1, &bar[b]);
+        } else {
+            tma_load_2d(base, &tmN, c0, 1, &bar[b]);                       // (u.grad)u -> P0
+            tma_load_2d(base + PS, &tmN, c0, 2 * d.Ny + 1, &bar[b]);      // (u.grad)w -> P1
+            tma_load_2d(base + 2 * PS, &tmN, c0, d.Ny + 1, &bar[b]);      // (u.grad)v -> P2
+            tma_load_2d(base + 3 * PS, &tmV, c0, 1, &bar[b]);             // v_t      -> P3
+            tma_load_2d(base + 4 * PS, &tmE, c0, 1, &bar[b]);             // eta_t    -> P4
+        }
+    };
+
     if (threadIdx.x == 0) {
-        mbar_init(&bar, 1);
+        mbar_init(&bar[0], 1);
+        mbar_init(&bar[1], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        s_item[0] = (int)atomicAdd(d.ypctr, 1u);
     }
     __syncthreads();
-    if (threadIdx.x == 0) mbar_arrive_expect_tx(&bar, (uint32_t)(nf * Ni) * rowbytes);
-    for (int it = threadIdx.x; it < nf * Ni; it += blockDim.x) {
-        const int f = it / Ni, r = it - f * Ni;
-        const double2* src;
-        double* dst;
-        if (derive_only) { src = f == 0 ? d.vt : d.et; dst = f == 0 ? P0 : P4; }
-        else {
-            src = f == 0 ? d.Nh : f == 1 ? d.Nh + 2 * d.S : f == 2 ? d.Nh + d.S : f == 3 ? d.vt : d.et;
-            dst = smy + (size_t)f * PS;
-        }
-        bulk_g2s(dst + (size_t)r * ld, src + pbase + (size_t)(r + 1) * rowstride, rowbytes, &bar);
-    }
+    int cur = s_item[0];
+    if (threadIdx.x == 0 && cur < nitems) issue(cur, 0);
 
-    // ---- own fragment elements: row i = 8 mt + g of both parities, columns col0 + 8 nt + 2t, +1 (one member)
+    // own fragment elements: row i = 8 mt + g of both parities, columns col0 + 8 nt + 2t, +1 (one member)
     const int i = 8 * mt + g, Ji = Ni - 1 - i;
     const bool sok = i < Kh, dok = i < Kho;
     const int col0 = 8 * NT * wn;
     const int offS = (sok ? i : 0) * ld + col0 + 2 * t, offD = (dok ? Ji : 0) * ld + col0 + 2 * t;
-    auto eokf = [&](int nt) { return (e0 + (col0 >> 1) + 4 * nt + t) < d.E; };
-    const size_t gS = pbase + (size_t)(i + 1) * rowstride + (col0 >> 1) + t;      // + 4 nt : natural row i
-    const size_t gD = pbase + (size_t)(Ji + 1) * rowstride + (col0 >> 1) + t;     // natural row J i
 
-    // ---- history of the nonlinear terms: hist = N0 after stage 0, N0 + 4 N1 after stage 1
-    double2 fhS[NT], fhD[NT], ghA[NT], ghB[NT];
-    if (!derive_only && stage > 0) {
-#pragma unroll
-        for (int nt = 0; nt < NT; ++nt) {
-            fhS[nt] = fhD[nt] = make_double2(0.0, 0.0);
-            if (eokf(nt)) {
-                if (sok) fhS[nt] = d.F0[gS + 4 * nt];
-                if (dok) fhD[nt] = d.F0[gD + 4 * nt];
-            }
+    for (int k = 0; cur < nitems; ++k) {
+        const int b = k & 1;
+        if (threadIdx.x == 0) {                              // hand out the next item and start its loads
+            const int nx = (int)atomicAdd(d.ypctr, 1u);
+            s_item[b ^ 1] = nx;
+            if (nx < nitems) issue(nx, b ^ 1);
         }
-#pragma unroll
-        for (int k = 0; k < NT; ++k) {
-            const int q = threadIdx.x + k * blockDim.x, ia = q / ET, e = q - ia * ET;
-            ghA[k] = ghB[k] = make_double2(0.0, 0.0);
-            if (ia < Kh && e < nvalid) {
-                ghA[k] = d.G0[pbase + (size_t)(ia + 1) * rowstride + e];
-                ghB[k] = d.G0[pbase + (size_t)(Ni - ia) * rowstride + e];
-            }
-        }
-    }
-    mbar_wait(&bar, 0);
+        const int p = 1 + cur / ntile_e, e0 = (cur % ntile_e) * ET;
+        const int n = p / d.nkz, mi = p % d.nkz;
+        const int mabs = mi < d.nzh ? mi : d.nkz - mi;
+        const double kx = d.kx[n], kz = d.kz[mi], alpha = kx * kx + kz * kz, ialpha = 1.0 / alpha;
+        const double* mA = d.matsP + (((size_t)hi * d.nkx * d.nzh + (size_t)n * d.nzh + mabs) * 6) * BB;
+        double* P0 = smy + (size_t)b * 5 * PS;
+        double* P1 = P0 + PS;
+        double* P2 = P1 + PS;
+        double* P3 = P2 + PS;
+        double* P4 = P3 + PS;
+        const size_t pbase = (size_t)p * d.E + e0;          // + (row + 1) * rowstride + member
+        const int nvalid = d.E - e0 < ET ? d.E - e0 : ET;
+        auto eokf = [&](int nt) { return (e0 + (col0 >> 1) + 4 * nt + t) < d.E; };
+        const size_t gS = pbase + (size_t)(i + 1) * rowstride + (col0 >> 1) + t;      // + 4 nt : natural row i
+        const size_t gD = pbase + (size_t)(Ji + 1) * rowstride + (col0 >> 1) + t;     // natural row J i
 
-    double accS[NT][2], accD[NT][2];
-    if (!derive_only) {
-        // ---- A (element-wise, in place): natural rows (ia, J ia) -> parity rows; H = i kx Nu + i kz Nw -> P0,
-        //      G = i kz Nu - i kx Nw (Eq. 5), RK3 combination, 2 eta_t - h dt Gc -> P1, Nv -> P2, 2 v_t -> P3, eta_t -> P4
+        // history of the nonlinear terms: hist = N0 after stage 0, N0 + 4 N1 after stage 1
+        double2 fhS[NT], fhD[NT], ghA[NT], ghB[NT];
+        if (!derive_only && stage > 0) {
 #pragma unroll
-        for (int k = 0; k < NT; ++k) {
-            const int q = threadIdx.x + k * blockDim.x, ia = q / ET, e = q - ia * ET;
-            if (ia >= Kh) continue;
-            const int ib = Ni - 1 - ia;
-            double* a0 = P0 + ia * ld + 2 * e;
-            double* b0 = P0 + ib * ld + 2 * e;
-            const double2 nuA = ld2(a0), nuB = ld2(b0), nwA = ld2(a0 + PS), nwB = ld2(b0 + PS);
-            const double2 nvA = ld2(a0 + 2 * PS), nvB = ld2(b0 + 2 * PS), vtA = ld2(a0 + 3 * PS), vtB = ld2(b0 + 3 * PS);
-            const double2 etA = ld2(a0 + 4 * PS), etB = ld2(b0 + 4 * PS);
-            const double2 HA = make_double2(-kx * nuA.y - kz * nwA.y, kx * nuA.x + kz * nwA.x);
-            const double2 HB = make_double2(-kx * nuB.y - kz * nwB.y, kx * nuB.x + kz * nwB.x);
-            const double2 GA = make_double2(-kz * nuA.y + kx * nwA.y, kz * nuA.x - kx * nwA.x);
-            const double2 GB = make_double2(-kz * nuB.y + kx * nwB.y, kz * nuB.x - kx * nwB.x);
-            double2 GcA, GcB;
-            const bool eok = e < nvalid;
-            const size_t giA = pbase + (size_t)(ia + 1) * rowstride + e, giB = pbase + (size_t)(ib + 1) * rowstride + e;
-            if (stage == 0) {
-                GcA = GA; GcB = GB;
-                if (eok) { d.G0[giA] = GA; d.G0[giB] = GB; }
-            } else if (stage == 1) {
-                GcA = make_double2(2.0 * GA.x - ghA[k].x, 2.0 * GA.y - ghA[k].y);
-                GcB = make_double2(2.0 * GB.x - ghB[k].x, 2.0 * GB.y - ghB[k].y);
-                if (eok) {
-                    d.G0[giA] = make_double2(ghA[k].x + 4.0 * GA.x, ghA[k].y + 4.0 * GA.y);
-                    d.G0[giB] = make_double2(ghB[k].x + 4.0 * GB.x, ghB[k].y + 4.0 * GB.y);
+            for (int nt = 0; nt < NT; ++nt) {
+                fhS[nt] = fhD[nt] = make_double2(0.0, 0.0);
+                if (eokf(nt)) {
+                    if (sok) fhS[nt] = d.F0[gS + 4 * nt];
+                    if (dok) fhD[nt] = d.F0[gD + 4 * nt];
                 }
-            } else {
-                GcA = make_double2((ghA[k].x + GA.x) / 6.0, (ghA[k].y + GA.y) / 6.0);
-                GcB = make_double2((ghB[k].x + GB.x) / 6.0, (ghB[k].y + GB.y) / 6.0);
             }
-            const double2 rA = make_double2(2.0 * etA.x - hdt * GcA.x, 2.0 * etA.y - hdt * GcA.y);
-            const double2 rB = make_double2(2.0 * etB.x - hdt * GcB.x, 2.0 * etB.y - hdt * GcB.y);
-            st2(a0, make_double2(HA.x + HB.x, HA.y + HB.y));
-            st2(a0 + PS, make_double2(rA.x + rB.x, rA.y + rB.y));
-            st2(a0 + 2 * PS, make_double2(nvA.x + nvB.x, nvA.y + nvB.y));
-            st2(a0 + 3 * PS, make_double2(2.0 * (vtA.x + vtB.x), 2.0 * (vtA.y + vtB.y)));
-            st2(a0 + 4 * PS, make_double2(etA.x + etB.x, etA.y + etB.y));
-            if (ib != ia) {
-                st2(b0, make_double2(HA.x - HB.x, HA.y - HB.y));
-                st2(b0 + PS, make_double2(rA.x - rB.x, rA.y - rB.y));
-                st2(b0 + 2 * PS, make_double2(nvA.x - nvB.x, nvA.y - nvB.y));
-                st2(b0 + 3 * PS, make_double2(2.0 * (vtA.x - vtB.x), 2.0 * (vtA.y - vtB.y)));
-                st2(b0 + 4 * PS, make_double2(etA.x - etB.x, etA.y - etB.y));
+#pragma unroll
+            for (int kk = 0; kk < NT; ++kk) {
+                const int q = threadIdx.x + kk * blockDim.x, ia = q / ET, e = q - ia * ET;
+                ghA[kk] = ghB[kk] = make_double2(0.0, 0.0);
+                if (ia < Kh && e < nvalid) {
+                    ghA[kk] = d.G0[pbase + (size_t)(ia + 1) * rowstride + e];
+                    ghB[kk] = d.G0[pbase + (size_t)(Ni - ia) * rowstride + e];
+                }
             }
         }
-        __syncthreads();
-        // ---- B: F = -alpha Nv - D H (Eq. 4 with Eq. 10's sign), RK3 combination; -h dt Fc -> P2
-        zero_acc<NT>(accS); zero_acc<NT>(accD);
-        gemm_blk<NT, KS2T, true>(accS, Dsd, P0, KS2, mt, lane, ld, Ni, col0);
-        gemm_blk<NT, KS2T, false>(accD, Dds, P0, KS2, mt, lane, ld, Ni, col0);
-#pragma unroll
-        for (int nt = 0; nt < NT; ++nt) {
-            double2 FS = make_double2(0.0, 0.0), FD = make_double2(0.0, 0.0);
-            if (sok) { const double2 nv = ld2(P2 + offS + 8 * nt); FS = make_double2(-alpha * nv.x - accS[nt][0], -alpha * nv.y - accS[nt][1]); }
-            if (dok) { const double2 nv = ld2(P2 + offD + 8 * nt); FD = make_double2(-alpha * nv.x - accD[nt][0], -alpha * nv.y - accD[nt][1]); }
-            // natural rows: F(i) = (FS + FD)/2, F(Ji) = (FS - FD)/2
-            const double2 FA = make_double2(0.5 * (FS.x + FD.x), 0.5 * (FS.y + FD.y));
-            const double2 FB = make_double2(0.5 * (FS.x - FD.x), 0.5 * (FS.y - FD.y));
-            double2 cA, cB;
-            const bool eok = eokf(nt);
-            if (stage == 0) {
-                cA = FA; cB = FB;
-                if (eok && sok) d.F0[gS + 4 * nt] = FA;
-                if (eok && dok) d.F0[gD + 4 * nt] = FB;
-            } else if (stage == 1) {
-                cA = make_double2(2.0 * FA.x - fhS[nt].x, 2.0 * FA.y - fhS[nt].y);
-                cB = make_double2(2.0 * FB.x - fhD[nt].x, 2.0 * FB.y - fhD[nt].y);
-                if (eok && sok) d.F0[gS + 4 * nt] = make_double2(fhS[nt].x + 4.0 * FA.x, fhS[nt].y + 4.0 * FA.y);
-                if (eok && dok) d.F0[gD + 4 * nt] = make_double2(fhD[nt].x + 4.0 * FB.x, fhD[nt].y + 4.0 * FB.y);
-            } else {
-                cA = make_double2((fhS[nt].x + FA.x) / 6.0, (fhS[nt].y + FA.y) / 6.0);
-                cB = make_double2((fhD[nt].x + FB.x) / 6.0, (fhD[nt].y + FB.y) / 6.0);
+        mbar_wait(&bar[b], (k >> 1) & 1);
+
+        double accS[NT][2], accD[NT][2];
+        if (!derive_only) {
+            // ---- A (element-wise, in place): natural rows (ia, J ia) -> parity rows; H = i kx Nu + i kz Nw -> P0,
+            //      G = i kz Nu - i kx Nw (Eq. 5), RK3 combination, 2 eta_t - h dt Gc -> P1, Nv -> P2, 2 v_t -> P3, eta_t -> P4
+    #pragma unroll
+            for (int kk = 0; kk < NT; ++kk) {
+                const int q = threadIdx.x + kk * blockDim.x, ia = q / ET, e = q - ia * ET;
+                if (ia >= Kh) continue;
+                const int ib = Ni - 1 - ia;
+                double* a0 = P0 + ia * ld + 2 * e;
+                double* b0 = P0 + ib * ld + 2 * e;
+                const double2 nuA = ld2(a0), nuB = ld2(b0), nwA = ld2(a0 + PS), nwB = ld2(b0 + PS);
+                const double2 nvA = ld2(a0 + 2 * PS), nvB = ld2(b0 + 2 * PS), vtA = ld2(a0 + 3 * PS), vtB = ld2(b0 + 3 * PS);
+                const double2 etA = ld2(a0 + 4 * PS), etB = ld2(b0 + 4 * PS);
+                const double2 HA = make_double2(-kx * nuA.y - kz * nwA.y, kx * nuA.x + kz * nwA.x);
+                const double2 HB = make_double2(-kx * nuB.y - kz * nwB.y, kx * nuB.x + kz * nwB.x);
+                const double2 GA = make_double2(-kz * nuA.y + kx * nwA.y, kz * nuA.x - kx * nwA.x);
+                const double2 GB = make_double2(-kz * nuB.y + kx * nwB.y, kz * nuB.x - kx * nwB.x);
+                double2 GcA, GcB;
+                const bool eok = e < nvalid;
+                const size_t giA = pbase + (size_t)(ia + 1) * rowstride + e, giB = pbase + (size_t)(ib + 1) * rowstride + e;
+                if (stage == 0) {
+                    GcA = GA; GcB = GB;
+                    if (eok) { d.G0[giA] = GA; d.G0[giB] = GB; }
+                } else if (stage == 1) {
+                    GcA = make_double2(2.0 * GA.x - ghA[kk].x, 2.0 * GA.y - ghA[kk].y);
+                    GcB = make_double2(2.0 * GB.x - ghB[kk].x, 2.0 * GB.y - ghB[kk].y);
+                    if (eok) {
+                        d.G0[giA] = make_double2(ghA[kk].x + 4.0 * GA.x, ghA[kk].y + 4.0 * GA.y);
+                        d.G0[giB] = make_double2(ghB[kk].x + 4.0 * GB.x, ghB[kk].y + 4.0 * GB.y);
+                    }
+                } else {
+                    GcA = make_double2((ghA[kk].x + GA.x) / 6.0, (ghA[kk].y + GA.y) / 6.0);
+                    GcB = make_double2((ghB[kk].x + GB.x) / 6.0, (ghB[kk].y + GB.y) / 6.0);
+                }
+                const double2 rA = make_double2(2.0 * etA.x - hdt * GcA.x, 2.0 * etA.y - hdt * GcA.y);
+                const double2 rB = make_double2(2.0 * etB.x - hdt * GcB.x, 2.0 * etB.y - hdt * GcB.y);
+                st2(a0, make_double2(HA.x + HB.x, HA.y + HB.y));
+                st2(a0 + PS, make_double2(rA.x + rB.x, rA.y + rB.y));
+                st2(a0 + 2 * PS, make_double2(nvA.x + nvB.x, nvA.y + nvB.y));
+                st2(a0 + 3 * PS, make_double2(2.0 * (vtA.x + vtB.x), 2.0 * (vtA.y + vtB.y)));
+                st2(a0 + 4 * PS, make_double2(etA.x + etB.x, etA.y + etB.y));
+                if (ib != ia) {
+                    st2(b0, make_double2(HA.x - HB.x, HA.y - HB.y));
+                    st2(b0 + PS, make_double2(rA.x - rB.x, rA.y - rB.y));
+                    st2(b0 + 2 * PS, make_double2(nvA.x - nvB.x, nvA.y - nvB.y));
+                    st2(b0 + 3 * PS, make_double2(2.0 * (vtA.x - vtB.x), 2.0 * (vtA.y - vtB.y)));
+                    st2(b0 + 4 * PS, make_double2(etA.x - etB.x, etA.y - etB.y));
+                }
             }
-            if (!dok) cB = cA;                              // middle row of an odd Ni: s = 2 x
-            if (sok) st2(P2 + offS + 8 * nt, make_double2(-hdt * (cA.x + cB.x), -hdt * (cA.y + cB.y)));
-            if (dok) st2(P2 + offD + 8 * nt, make_double2(-hdt * (cA.x - cB.x), -hdt * (cA.y - cB.y)));
+            __syncthreads();
+            // ---- B: F = -alpha Nv - D H (Eq. 4 with Eq. 10's sign), RK3 combination; -h dt Fc -> P2
+            zero_acc<NT>(accS); zero_acc<NT>(accD);
+            gemm2<NT, KS2T, true, false>(accS, accD, Dsd, Dds, P0, P0, KS2, mt, lane, ld, Ni, col0);
+    #pragma unroll
+            for (int nt = 0; nt < NT; ++nt) {
+                double2 FS = make_double2(0.0, 0.0), FD = make_double2(0.0, 0.0);
+                if (sok) { const double2 nv = ld2(P2 + offS + 8 * nt); FS = make_double2(-alpha * nv.x - accS[nt][0], -alpha * nv.y - accS[nt][1]); }
+                if (dok) { const double2 nv = ld2(P2 + offD + 8 * nt); FD = make_double2(-alpha * nv.x - accD[nt][0], -alpha * nv.y - accD[nt][1]); }
+                // natural rows: F(i) = (FS + FD)/2, F(Ji) = (FS - FD)/2
+                const double2 FA = make_double2(0.5 * (FS.x + FD.x), 0.5 * (FS.y + FD.y));
+                const double2 FB = make_double2(0.5 * (FS.x - FD.x), 0.5 * (FS.y - FD.y));
+                double2 cA, cB;
+                const bool eok = eokf(nt);
+                if (stage == 0) {
+                    cA = FA; cB = FB;
+                    if (eok && sok) d.F0[gS + 4 * nt] = FA;
+                    if (eok && dok) d.F0[gD + 4 * nt] = FB;
+                } else if (stage == 1) {
+                    cA = make_double2(2.0 * FA.x - fhS[nt].x, 2.0 * FA.y - fhS[nt].y);
+                    cB = make_double2(2.0 * FB.x - fhD[nt].x, 2.0 * FB.y - fhD[nt].y);
+                    if (eok && sok) d.F0[gS + 4 * nt] = make_double2(fhS[nt].x + 4.0 * FA.x, fhS[nt].y + 4.0 * FA.y);
+                    if (eok && dok) d.F0[gD + 4 * nt] = make_double2(fhD[nt].x + 4.0 * FB.x, fhD[nt].y + 4.0 * FB.y);
+                } else {
+                    cA = make_double2((fhS[nt].x + FA.x) / 6.0, (fhS[nt].y + FA.y) / 6.0);
+                    cB = make_double2((fhD[nt].x + FB.x) / 6.0, (fhD[nt].y + FB.y) / 6.0);
+                }
+                if (!dok) cB = cA;                              // middle row of an odd Ni: s = 2 x
+                if (sok) st2(P2 + offS + 8 * nt, make_double2(-hdt * (cA.x + cB.x), -hdt * (cA.y + cB.y)));
+                if (dok) st2(P2 + offD + 8 * nt, make_double2(-hdt * (cA.x - cB.x), -hdt * (cA.y - cB.y)));
+            }
+            __syncthreads();
+            // ---- C: v' = Ainv (2 v_t) + AD (-h dt Fc) - v_t (Eq. 12) -> global, P0 ; eta' = Sinv P1 - eta_t (Eq. 13) -> P4
+            zero_acc<NT>(accS); zero_acc<NT>(accD);
+            gemm2<NT, KS2T, false, true>(accS, accD, mA, mA + BB, P3, P3, KS2, mt, lane, ld, Ni, col0);
+            gemm2<NT, KS2T, false, true>(accS, accD, mA + 2 * BB, mA + 3 * BB, P2, P2, KS2, mt, lane, ld, Ni, col0);
+            double acc2S[NT][2], acc2D[NT][2];
+            zero_acc<NT>(acc2S); zero_acc<NT>(acc2D);
+            gemm2<NT, KS2T, false, true>(acc2S, acc2D, mA + 4 * BB, mA + 5 * BB, P1, P1, KS2, mt, lane, ld, Ni, col0);
+    #pragma unroll
+            for (int nt = 0; nt < NT; ++nt) {
+                double2 vS = make_double2(0.0, 0.0), vD = vS, eS = vS, eD = vS;
+                if (sok) {
+                    const double2 v2 = ld2(P3 + offS + 8 * nt), et = ld2(P4 + offS + 8 * nt);
+                    vS = make_double2(accS[nt][0] - 0.5 * v2.x, accS[nt][1] - 0.5 * v2.y);
+                    eS = make_double2(acc2S[nt][0] - et.x, acc2S[nt][1] - et.y);
+                    st2(P0 + offS + 8 * nt, vS);
+                    st2(P4 + offS + 8 * nt, eS);
+                }
+                if (dok) {
+                    const double2 v2 = ld2(P3 + offD + 8 * nt), et = ld2(P4 + offD + 8 * nt);
+                    vD = make_double2(accD[nt][0] - 0.5 * v2.x, accD[nt][1] - 0.5 * v2.y);
+                    eD = make_double2(acc2D[nt][0] - et.x, acc2D[nt][1] - et.y);
+                    st2(P0 + offD + 8 * nt, vD);
+                    st2(P4 + offD + 8 * nt, eD);
+                }
+                if (eokf(nt)) {
+                    if (sok) {
+                        vout[gS + 4 * nt] = make_double2(0.5 * (vS.x + vD.x), 0.5 * (vS.y + vD.y));
+                        if (stage == 2) d.et[gS + 4 * nt] = make_double2(0.5 * (eS.x + eD.x), 0.5 * (eS.y + eD.y));
+                    }
+                    if (dok) {
+                        vout[gD + 4 * nt] = make_double2(0.5 * (vS.x - vD.x), 0.5 * (vS.y - vD.y));
+                        if (stage == 2) d.et[gD + 4 * nt] = make_double2(0.5 * (eS.x - eD.x), 0.5 * (eS.y - eD.y));
+                    }
+                }
+            }
+            __syncthreads();
+        } else {
+            // parity transform of v_t (P0) and eta_t (P4) in place
+    #pragma unroll
+            for (int kk = 0; kk < NT; ++kk) {
+                const int q = threadIdx.x + kk * blockDim.x, ia = q / ET, e = q - ia * ET;
+                if (ia >= Kh) continue;
+                const int ib = Ni - 1 - ia;
+                double* a0 = P0 + ia * ld + 2 * e;
+                double* b0 = P0 + ib * ld + 2 * e;
+                const double2 vA = ld2(a0), vB = ld2(b0), eA = ld2(a0 + 4 * PS), eB = ld2(b0 + 4 * PS);
+                st2(a0, make_double2(vA.x + vB.x, vA.y + vB.y));
+                st2(a0 + 4 * PS, make_double2(eA.x + eB.x, eA.y + eB.y));
+                if (ib != ia) {
+                    st2(b0, make_double2(vA.x - vB.x, vA.y - vB.y));
+                    st2(b0 + 4 * PS, make_double2(eA.x - eB.x, eA.y - eB.y));
+                }
+            }
+            __syncthreads();
         }
-        __syncthreads();
-        // ---- C: v' = Ainv (2 v_t) + AD (-h dt Fc) - v_t (Eq. 12) -> global, P0 ; eta' = Sinv P1 - eta_t (Eq. 13) -> P4
+        // ---- D: dv/dy = D v' ; u = (i kx Dv - i kz eta)/alpha, w = (i kz Dv + i kx eta)/alpha (Eq. 17-18) -> global, P2, P3
         zero_acc<NT>(accS); zero_acc<NT>(accD);
-        gemm_blk<NT, KS2T, false>(accS, mA, P3, KS2, mt, lane, ld, Ni, col0);
-        gemm_blk<NT, KS2T, true>(accD, mA + BB, P3, KS2, mt, lane, ld, Ni, col0);
-        gemm_blk<NT, KS2T, false>(accS, mA + 2 * BB, P2, KS2, mt, lane, ld, Ni, col0);
-        gemm_blk<NT, KS2T, true>(accD, mA + 3 * BB, P2, KS2, mt, lane, ld, Ni, col0);
-        double acc2S[NT][2], acc2D[NT][2];
-        zero_acc<NT>(acc2S); zero_acc<NT>(acc2D);
-        gemm_blk<NT, KS2T, false>(acc2S, mA + 4 * BB, P1, KS2, mt, lane, ld, Ni, col0);
-        gemm_blk<NT, KS2T, true>(acc2D, mA + 5 * BB, P1, KS2, mt, lane, ld, Ni, col0);
-#pragma unroll
+        gemm2<NT, KS2T, true, false>(accS, accD, Dsd, Dds, P0, P0, KS2, mt, lane, ld, Ni, col0);
+    #pragma unroll
         for (int nt = 0; nt < NT; ++nt) {
-            double2 vS = make_double2(0.0, 0.0), vD = vS, eS = vS, eD = vS;
+            double2 uS = make_double2(0.0, 0.0), uD = uS, wS = uS, wD = uS;
             if (sok) {
-                const double2 v2 = ld2(P3 + offS + 8 * nt), et = ld2(P4 + offS + 8 * nt);
-                vS = make_double2(accS[nt][0] - 0.5 * v2.x, accS[nt][1] - 0.5 * v2.y);
-                eS = make_double2(acc2S[nt][0] - et.x, acc2S[nt][1] - et.y);
-                st2(P0 + offS + 8 * nt, vS);
-                st2(P4 + offS + 8 * nt, eS);
+                const double2 en = ld2(P4 + offS + 8 * nt);
+                uS = make_double2((-kx * accS[nt][1] + kz * en.y) * ialpha, (kx * accS[nt][0] - kz * en.x) * ialpha);
+                wS = make_double2((-kz * accS[nt][1] - kx * en.y) * ialpha, (kz * accS[nt][0] + kx * en.x) * ialpha);
+                st2(P2 + offS + 8 * nt, uS);
+                st2(P3 + offS + 8 * nt, wS);
             }
             if (dok) {
-                const double2 v2 = ld2(P3 + offD + 8 * nt), et = ld2(P4 + offD + 8 * nt);
-                vD = make_double2(accD[nt][0] - 0.5 * v2.x, accD[nt][1] - 0.5 * v2.y);
-                eD = make_double2(acc2D[nt][0] - et.x, acc2D[nt][1] - et.y);
-                st2(P0 + offD + 8 * nt, vD);
-                st2(P4 + offD + 8 * nt, eD);
+                const double2 en = ld2(P4 + offD + 8 * nt);
+                uD = make_double2((-kx * accD[nt][1] + kz * en.y) * ialpha, (kx * accD[nt][0] - kz * en.x) * ialpha);
+                wD = make_double2((-kz * accD[nt][1] - kx * en.y) * ialpha, (kz * accD[nt][0] + kx * en.x) * ialpha);
+                st2(P2 + offD + 8 * nt, uD);
+                st2(P3 + offD + 8 * nt, wD);
             }
             if (eokf(nt)) {
                 if (sok) {
-                    vout[gS + 4 * nt] = make_double2(0.5 * (vS.x + vD.x), 0.5 * (vS.y + vD.y));
-                    if (stage == 2) d.et[gS + 4 * nt] = make_double2(0.5 * (eS.x + eD.x), 0.5 * (eS.y + eD.y));
+                    d.uh[gS + 4 * nt] = make_double2(0.5 * (uS.x + uD.x), 0.5 * (uS.y + uD.y));
+                    d.wh[gS + 4 * nt] = make_double2(0.5 * (wS.x + wD.x), 0.5 * (wS.y + wD.y));
                 }
                 if (dok) {
-                    vout[gD + 4 * nt] = make_double2(0.5 * (vS.x - vD.x), 0.5 * (vS.y - vD.y));
-                    if (stage == 2) d.et[gD + 4 * nt] = make_double2(0.5 * (eS.x - eD.x), 0.5 * (eS.y - eD.y));
+                    d.uh[gD + 4 * nt] = make_double2(0.5 * (uS.x - uD.x), 0.5 * (uS.y - uD.y));
+                    d.wh[gD + 4 * nt] = make_double2(0.5 * (wS.x - wD.x), 0.5 * (wS.y - wD.y));
                 }
             }
         }
         __syncthreads();
-    } else {
-        // parity transform of v_t (P0) and eta_t (P4) in place
-#pragma unroll
-        for (int k = 0; k < NT; ++k) {
-            const int q = threadIdx.x + k * blockDim.x, ia = q / ET, e = q - ia * ET;
-            if (ia >= Kh) continue;
-            const int ib = Ni - 1 - ia;
-            double* a0 = P0 + ia * ld + 2 * e;
-            double* b0 = P0 + ib * ld + 2 * e;
-            const double2 vA = ld2(a0), vB = ld2(b0), eA = ld2(a0 + 4 * PS), eB = ld2(b0 + 4 * PS);
-            st2(a0, make_double2(vA.x + vB.x, vA.y + vB.y));
-            st2(a0 + 4 * PS, make_double2(eA.x + eB.x, eA.y + eB.y));
-            if (ib != ia) {
-                st2(b0, make_double2(vA.x - vB.x, vA.y - vB.y));
-                st2(b0 + 4 * PS, make_double2(eA.x - eB.x, eA.y - eB.y));
+        // ---- E: du/dy, dw/dy
+        {
+            double a2S[NT][2], a2D[NT][2];
+            zero_acc<NT>(accS); zero_acc<NT>(accD); zero_acc<NT>(a2S); zero_acc<NT>(a2D);
+            gemm2<NT, KS2T, true, false>(accS, accD, Dsd, Dds, P2, P2, KS2, mt, lane, ld, Ni, col0);
+            gemm2<NT, KS2T, true, false>(a2S, a2D, Dsd, Dds, P3, P3, KS2, mt, lane, ld, Ni, col0);
+    #pragma unroll
+            for (int nt = 0; nt < NT; ++nt) {
+                if (!eokf(nt)) continue;
+                if (sok) {
+                    d.duh[gS + 4 * nt] = make_double2(0.5 * (accS[nt][0] + accD[nt][0]), 0.5 * (accS[nt][1] + accD[nt][1]));
+                    d.dwh[gS + 4 * nt] = make_double2(0.5 * (a2S[nt][0] + a2D[nt][0]), 0.5 * (a2S[nt][1] + a2D[nt][1]));
+                }
+                if (dok) {
+                    d.duh[gD + 4 * nt] = make_double2(0.5 * (accS[nt][0] - accD[nt][0]), 0.5 * (accS[nt][1] - accD[nt][1]));
+                    d.dwh[gD + 4 * nt] = make_double2(0.5 * (a2S[nt][0] - a2D[nt][0]), 0.5 * (a2S[nt][1] - a2D[nt][1]));
+                }
             }
         }
-        __syncthreads();
+        __syncthreads();                                     // every warp is done with panel set b
+        cur = s_item[b ^ 1];
     }
-    // ---- D: dv/dy = D v' ; u = (i kx Dv - i kz eta)/alpha, w = (i kz Dv + i kx eta)/alpha (Eq. 17-18) -> global, P2, P3
-    zero_acc<NT>(accS); zero_acc<NT>(accD);
-    gemm_blk<NT, KS2T, true>(accS, Dsd, P0, KS2, mt, lane, ld, Ni, col0);
-    gemm_blk<NT, KS2T, false>(accD, Dds, P0, KS2, mt, lane, ld, Ni, col0);
-#pragma unroll
-    for (int nt = 0; nt < NT; ++nt) {
-        double2 uS = make_double2(0.0, 0.0), uD = uS, wS = uS, wD = uS;
-        if (sok) {
-            const double2 en = ld2(P4 + offS + 8 * nt);
-            uS = make_double2((-kx * accS[nt][1] + kz * en.y) * ialpha, (kx * accS[nt][0] - kz * en.x) * ialpha);
-            wS = make_double2((-kz * accS[nt][1] - kx * en.y) * ialpha, (kz * accS[nt][0] + kx * en.x) * ialpha);
-            st2(P2 + offS + 8 * nt, uS);
-            st2(P3 + offS + 8 * nt, wS);
-        }
-        if (dok) {
-            const double2 en = ld2(P4 + offD + 8 * nt);
-            uD = make_double2((-kx * accD[nt][1] + kz * en.y) * ialpha, (kx * accD[nt][0] - kz * en.x) * ialpha);
-            wD = make_double2((-kz * accD[nt][1] - kx * en.y) * ialpha, (kz * accD[nt][0] + kx * en.x) * ialpha);
-            st2(P2 + offD + 8 * nt, uD);
-            st2(P3 + offD + 8 * nt, wD);
-        }
-        if (eokf(nt)) {
-            if (sok) {
-                d.uh[gS + 4 * nt] = make_double2(0.5 * (uS.x + uD.x), 0.5 * (uS.y + uD.y));
-                d.wh[gS + 4 * nt] = make_double2(0.5 * (wS.x + wD.x), 0.5 * (wS.y + wD.y));
-            }
-            if (dok) {
-                d.uh[gD + 4 * nt] = make_double2(0.5 * (uS.x - uD.x), 0.5 * (uS.y - uD.y));
-                d.wh[gD + 4 * nt] = make_double2(0.5 * (wS.x - wD.x), 0.5 * (wS.y - wD.y));
-            }
-        }
-    }
-    __syncthreads();
-    // ---- E: du/dy, dw/dy
-    {
-        double a2S[NT][2], a2D[NT][2];
-        zero_acc<NT>(accS); zero_acc<NT>(accD); zero_acc<NT>(a2S); zero_acc<NT>(a2D);
-        gemm_blk<NT, KS2T, true>(accS, Dsd, P2, KS2, mt, lane, ld, Ni, col0);
-        gemm_blk<NT, KS2T, false>(accD, Dds, P2, KS2, mt, lane, ld, Ni, col0);
-        gemm_blk<NT, KS2T, true>(a2S, Dsd, P3, KS2, mt, lane, ld, Ni, col0);
-        gemm_blk<NT, KS2T, false>(a2D, Dds, P3, KS2, mt, lane, ld, Ni, col0);
-#pragma unroll
-        for (int nt = 0; nt < NT; ++nt) {
-            if (!eokf(nt)) continue;
-            if (sok) {
-                d.duh[gS + 4 * nt] = make_double2(0.5 * (accS[nt][0] + accD[nt][0]), 0.5 * (accS[nt][1] + accD[nt][1]));
-                d.dwh[gS + 4 * nt] = make_double2(0.5 * (a2S[nt][0] + a2D[nt][0]), 0.5 * (a2S[nt][1] + a2D[nt][1]));
-            }
-            if (dok) {
-                d.duh[gD + 4 * nt] = make_double2(0.5 * (accS[nt][0] - accD[nt][0]), 0.5 * (accS[nt][1] - accD[nt][1]));
-                d.dwh[gD + 4 * nt] = make_double2(0.5 * (a2S[nt][0] - a2D[nt][0]), 0.5 * (a2S[nt][1] - a2D[nt][1]));
-            }
-        }
+    // the last CTA to leave re-arms the work counter for the next launch (launches are stream-ordered)
+    if (threadIdx.x == 0) {
+        __threadfence();
+        const unsigned done = atomicAdd(d.ypctr + 1, 1u);
+        if (done == gridDim.x - 1) { d.ypctr[0] = 0u; d.ypctr[1] = 0u; __threadfence(); }
     }
 }
 
@@ -578,32 +613,71 @@ __global__ void k_diag_rows(DnsDev d, const double* __restrict__ part, double t)
 }  // namespace
 
 size_t dns_ypair_smem(int Ni, int Ny, int ET) {
-    const size_t panels = (size_t)5 * Ni * (2 * ET + 4) * sizeof(double), mean = (size_t)6 * Ny * 8 * sizeof(double);
+    const size_t ps = (((size_t)Ni * (2 * ET + 4) + 15) & ~(size_t)15) * sizeof(double);
+    const size_t panels = 2 * 5 * ps, mean = (size_t)6 * Ny * 8 * sizeof(double);
     return panels > mean ? panels : mean;
 }
 
-template <int NT, int NWN> static void ypair_launch(dns_plan* p, int stage, int derive_only) {
+// TMA descriptors of the per-pair kernel's inputs: 2-D views [rows][2 P E doubles] of the spectral arrays with a
+// box of Ni rows x (2 ET + 4) doubles, i.e. exactly one padded shared-memory panel.  Encoded at dns_plan_bind.
+int dns_ypair_encode_maps(dns_plan* p) {
+    typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    static encode_fn encode = nullptr;
+    if (!encode) {
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) != cudaSuccess || !fn) return DNS_ECUDA;
+        encode = reinterpret_cast<encode_fn>(fn);
+    }
     const DnsDev& d = p->d;
-    const int KS2 = d.Kp >> 3, ET = 4 * NT * NWN;
+    static_assert(sizeof(CUtensorMap) == sizeof(p->tmaps[0]), "tensor map storage");
+    struct Src { void* ptr; cuuint64_t rows; } src[3] = {{d.Nh, (cuuint64_t)3 * d.Ny}, {d.vt, (cuuint64_t)d.Ny}, {d.et, (cuuint64_t)d.Ny}};
+    for (int i = 0; i < 3; ++i) {
+        const cuuint64_t dims[2] = {(cuuint64_t)2 * d.P * d.E, src[i].rows};
+        const cuuint64_t strides[1] = {(cuuint64_t)d.P * d.E * sizeof(double2)};
+        const cuuint32_t box[2] = {(cuuint32_t)(2 * p->ETy + 4), (cuuint32_t)d.Ni};
+        const cuuint32_t estr[2] = {1, 1};
+        CUresult r = encode(reinterpret_cast<CUtensorMap*>(&p->tmaps[i]), CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, src[i].ptr, dims,
+                            strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                            CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) return DNS_ECUDA;
+    }
+    return DNS_OK;
+}
+
+template <int NT, int NWN, int K> static void ypair_launch_k(dns_plan* p, int stage, int derive_only) {
+    const DnsDev& d = p->d;
+    const int KS2 = d.Kp >> 3, ET = 4 * NT * NWN, threads = 32 * KS2 * NWN;
     const int nmean = (d.E + 7) / 8;
-    const unsigned grid = (unsigned)(nmean + (d.P - 1) * ((d.E + ET - 1) / ET));
+    const int nitems = (d.P - 1) * ((d.E + ET - 1) / ET);
     const size_t smem = dns_ypair_smem(d.Ni, d.Ny, ET);
-#define LAUNCH(K)                                                                                     \
-    {                                                                                                 \
-        auto kern = k_ypair<NT, NWN, K>;                                                              \
-        cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);           \
-        cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared); \
-        static const int nomean = getenv("DNS_NOMEAN") ? 8 : 0;                                       \
-        kern<<<grid, 32 * KS2 * NWN, smem, p->stream>>>(d, stage | nomean, derive_only, nmean);       \
+    auto kern = k_ypair<NT, NWN, K>;
+    if (p->ypair_grid == 0) {
+        cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+        int nb = 0, nsm = 0, dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, threads, smem);
+        if (nb < 1) nb = 1;
+        p->ypair_grid = nsm * nb;
     }
-    switch (KS2) {
-        case 2: LAUNCH(2) break;
-        case 3: LAUNCH(3) break;
-        case 4: LAUNCH(4) break;
-        case 6: LAUNCH(6) break;
-        default: LAUNCH(0) break;
+    int grid = nitems < p->ypair_grid ? nitems : p->ypair_grid;
+    if (grid < nmean) grid = nmean;
+    const CUtensorMap* tm = reinterpret_cast<const CUtensorMap*>(p->tmaps);
+    kern<<<grid, threads, smem, p->stream>>>(d, tm[0], tm[1], tm[2], stage, derive_only, nmean, nitems);
+}
+
+template <int NT, int NWN> static void ypair_launch(dns_plan* p, int stage, int derive_only) {
+    switch (p->d.Kp >> 3) {
+        case 2: ypair_launch_k<NT, NWN, 2>(p, stage, derive_only); break;
+        case 3: ypair_launch_k<NT, NWN, 3>(p, stage, derive_only); break;
+        case 4: ypair_launch_k<NT, NWN, 4>(p, stage, derive_only); break;
+        case 6: ypair_launch_k<NT, NWN, 6>(p, stage, derive_only); break;
+        default: ypair_launch_k<NT, NWN, 0>(p, stage, derive_only); break;
     }
-#undef LAUNCH
 }
 
 void launch_ypair(dns_plan* p, int stage, int derive_only) {
