@@ -102,13 +102,16 @@ def workload_counts(cfg, E):
     fz = 5.0 * Mz * lg(Mz)                      # flops of one complex length-Mz FFT
     fx = 5.0 * Mx * lg(Mx)
     nmat = nkx * (cfg.Nz // 2) - 1
+    Kh, Kho = (Ni + 1) // 2, Ni // 2
     return {
         "fft_z_inv": {"bytes": 5 * S + 8 * I, "flops": 8 * Ni * nkx * E * fz},
         "line_fft_x_products": {"bytes": 11 * I + Ni * Mz * E * 16.0, "flops": Ni * Mz * E * (8 * fx + 15.0 * Mx)},
         "fft_z_fwd": {"bytes": 3 * I + 3 * S, "flops": 3 * Ni * nkx * E * fz},
-        # reads Nu,Nv,Nw,v_t,eta_t (+ stored F,G), writes v', u, w, du, dw (+F,G / eta): ~13 fields + 3 matrices per pair
-        "ypair_dmma": {"bytes": 13 * S + 3 * Ni * Ni * 8.0 * nmat, "flops": 7 * 2.0 * Ni * Ni * 2 * E * (P - 1)},
-        "mean_flow": {"bytes": Ni * Mz * E * 16.0 + 12 * cfg.Ny * E * 8.0, "flops": 8.0 * cfg.Ny * cfg.Ny * E},
+        # reads Nu,Nv,Nw,v_t,eta_t (+ F,G history), writes v', u, w, du, dw (+ history / eta): ~13 fields, plus the
+        # parity-folded matrices (3 per pair, half size); flops of the 7 products in the reflection-parity basis.
+        # The mean flow (row a10) rides in the first CTAs of the same launch: its bytes are added here.
+        "ypair_dmma": {"bytes": 13 * S + 3 * (Kh * Kh + Kho * Kho) * 8.0 * nmat + Ni * Mz * E * 16.0 + 12 * cfg.Ny * E * 8.0,
+                       "flops": 7 * 2.0 * (Kh * Kh + Kho * Kho) * 2 * E * (P - 1)},
     }
 
 

@@ -47,7 +47,6 @@ size_t carve_workspace(dns_plan* p, void* base) {
     d.Ut = c.take<double>(NE);  d.Wt = c.take<double>(NE);  d.Us = c.take<double>(NE);  d.Ws = c.take<double>(NE);
     d.gamma = c.take<double>(d.E);  d.Qstar = c.take<double>(d.E);
     d.diag = c.take<double>((size_t)d.E * 6 + NE);
-    d.ypctr = c.take<unsigned int>(64);
     d.stage_io = c.take<double2>(2 * S + 2 * NE);
     return c.off;
 }
@@ -65,23 +64,17 @@ bool is_device_ptr(const void* q) {
 }
 
 void run_stage(dns_plan* p, int s, cudaEvent_t* ev) {
-    // ev (optional): 5 events bracketing the 4 kernel launches of the main stream.  The mean flow (row a10) needs
-    // only the plane sums written by the line kernel: it is forked onto the side stream and joined at the end.
+    // ev (optional): 5 events bracketing the 4 kernel launches (the mean flow rides inside the per-pair launch)
     const double2* vin = s == 0 ? p->d.vt : p->d.vs;
     if (ev) cudaEventRecord(ev[0], p->stream);
     launch_zinv(p, vin);
     if (ev) cudaEventRecord(ev[1], p->stream);
     launch_line(p);
-    cudaEventRecord(p->ev_fork, p->stream);
-    cudaStreamWaitEvent(p->side, p->ev_fork, 0);
-    launch_mean(p, s, 0, p->side);
-    cudaEventRecord(p->ev_join, p->side);
     if (ev) cudaEventRecord(ev[2], p->stream);
     launch_zfwd(p);
     if (ev) cudaEventRecord(ev[3], p->stream);
     launch_ypair(p, s, 0);
     if (ev) cudaEventRecord(ev[4], p->stream);
-    cudaStreamWaitEvent(p->stream, p->ev_join, 0);
 }
 
 }  // namespace
@@ -134,18 +127,15 @@ int dns_plan_create(dns_plan** out, int Nx, int Ny, int Nz, int E, double Re, do
     // member tiles
     p->ETf = pow2ceil(E) < 32 ? pow2ceil(E) : 32;
     d.Kp = (((d.Ni + 1) / 2 + 7) / 8) * 8;
-    // per-pair kernel: a warp owns 4 NT members; NT = 2 when the ensemble has them and at least 4 warps fit an SM
-    p->NTy = (E > 4 && dns_ypair_smem(d.Ni, 2) * 4 <= 226 * 1024) ? 2 : 1;
-    if (const char* s = getenv("DNS_NTY")) { int v = atoi(s); if (v == 1 || v == 2) p->NTy = v; }
-    if (dns_ypair_smem(d.Ni, p->NTy) > 226 * 1024) p->NTy = 1;
-    if (dns_ypair_smem(d.Ni, 1) > 226 * 1024) { delete p; return DNS_EINVAL; }
-    if (cudaStreamCreateWithFlags(&p->side, cudaStreamNonBlocking) != cudaSuccess ||
-        cudaEventCreateWithFlags(&p->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
-        cudaEventCreateWithFlags(&p->ev_join, cudaEventDisableTiming) != cudaSuccess) {
-        cudaGetLastError();
-        dns_plan_destroy(p);
-        return DNS_ECUDA;
-    }
+    int ETy = pow2ceil(E) < 16 ? pow2ceil(E) : 16;
+    if (ETy < 4) ETy = 4;
+    while (ETy > 4 && dns_ypair_smem(d.Ni, Ny, ETy) > 75 * 1024) ETy >>= 1;
+    if (const char* s = getenv("DNS_ETY")) { int v = atoi(s); if (v == 4 || v == 8 || v == 16) ETy = v; }
+    if (dns_ypair_smem(d.Ni, Ny, ETy) > 227 * 1024) { delete p; return DNS_EINVAL; }
+    p->ETy = ETy;
+    p->NTy = ETy >= 8 ? 2 : 1;
+    if (const char* s = getenv("DNS_NTY")) { int v = atoi(s); if ((v == 1 || v == 2 || v == 4) && 4 * v <= ETy) p->NTy = v; }
+    while (32 * (d.Kp / 8) * (ETy / (4 * p->NTy)) > 1024) p->NTy *= 2;
     int st = DNS_OK;
     try {
         st = dns_host_precompute(p);
@@ -196,8 +186,7 @@ int dns_set_state(dns_plan* p, const double* vhat, const double* etahat, const d
     launch_abi_to_internal(p, se, d.et);
     launch_normalise_state(p);
     launch_mean_in(p, sU, sW);
-    launch_ypair(p, 0, 1);          // derive u, w, du/dy, dw/dy of the initial state (Eq. 17-18)
-    launch_mean(p, 0, 1, p->stream);   // and their (0,0) column
+    launch_ypair(p, 0, 1);          // derive u, w, du/dy, dw/dy of the initial state (Eq. 17-18), incl. the (0,0) column
     p->has_state = true;
     p->nsteps_done = 0;
     e = cudaGetLastError();
@@ -324,9 +313,6 @@ int dns_launches_per_step(const dns_plan* p) { return p ? 3 * 4 : 0; }
 int dns_plan_destroy(dns_plan* p) {
     if (!p) return DNS_OK;
     for (void* q : p->owned) cudaFree(q);
-    if (p->side) cudaStreamDestroy(p->side);
-    if (p->ev_fork) cudaEventDestroy(p->ev_fork);
-    if (p->ev_join) cudaEventDestroy(p->ev_join);
     if (p->ev_init)
         for (auto& e : p->ev) cudaEventDestroy(e);
     delete p;

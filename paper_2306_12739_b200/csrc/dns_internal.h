@@ -42,7 +42,6 @@ struct DnsDev {
     double *Ut, *Wt, *Us, *Ws;      // mean profiles at t and at the current stage
     double *gamma, *Qstar; // [E]
     double* diag;          // [E][6] + scratch [Ny][E]
-    unsigned int* ypctr;   // [2] work counter / exit counter of the persistent per-pair kernel (zero between launches)
     double2* stage_io;     // staging for ABI-layout copies: 2 spectral fields
     size_t S;              // Ny*P*E
     size_t Isz;            // Ny*Mz*ntl*nkx*2^etl
@@ -57,12 +56,9 @@ struct dns_plan {
     DnsDev d{};
     double Lx = 0, Lz = 0;
     int R1x = 0, R2x = 0, R1z = 0, R2z = 0;   // four-step factorisations of Mx, Mz
-    int NTy = 0;                               // n-tiles (groups of 4 members) a warp of the per-pair kernel owns
+    int ETy = 0, NTy = 0;                      // member tile of the per-pair kernel, n-tiles per warp
     int ETf = 0;                               // member tile of the transform kernels
     int line_grid = 0;                         // persistent grid of the line kernel (set at first launch)
-    int ypair_grid = 0, ypair_warps = 0;       // persistent grid / warps per CTA of the per-pair kernel (set at first launch)
-    cudaStream_t side = nullptr;               // the mean-flow kernel runs here, under the per-pair kernel
-    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
     alignas(64) unsigned char tmaps[3][128];   // CUtensorMap of Nh, vt, et (encoded at dns_plan_bind)
     std::vector<void*> owned;                  // plan-owned device allocations
     void* workspace = nullptr;
@@ -85,8 +81,7 @@ void launch_zinv(dns_plan* p, const double2* vin);
 void launch_line(dns_plan* p);
 void launch_zfwd(dns_plan* p);
 void launch_ypair(dns_plan* p, int stage, int derive_only);
-size_t dns_ypair_smem(int Ni, int NT);
-void launch_mean(dns_plan* p, int stage, int derive_only, cudaStream_t stream);
+size_t dns_ypair_smem(int Ni, int Ny, int ET);
 int dns_ypair_encode_maps(dns_plan* p);
 void launch_abi_to_internal(dns_plan* p, const double2* src_abi, double2* dst);
 void launch_internal_to_abi(dns_plan* p, const double2* src, double2* dst_abi);

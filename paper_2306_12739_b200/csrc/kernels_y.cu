@@ -1,20 +1,15 @@
 // Wall-normal part of one stage (north_star subsystems (3), (4)).
-//   k_ypair : persistent WARPS walk over work items (one (kx,kz) pair, one group of 4 or 8 members).  Everything that
-//             couples only along y is chained in the warp's shared-memory panels: F,G assembly (Eq. 4-5), RK3
-//             combination,
-//             the precomputed-inverse solves of Eq. 12-13 for ALL members of the tile at once,
-//             dv/dy, the u,w reconstruction of Eq. 17-18 and du/dy, dw/dy.  The contractions run on the fp64
-//             tensor cores (DMMA.8x8x4; the only fp64 MMA shape sm_100a executes natively) in the
-//             REFLECTION-PARITY basis: with J the reversal y -> -y of the interior Gauss-Lobatto points, the
-//             Chebyshev matrix obeys J D J = -D and every solve matrix J M J = M, so in the variables
-//             s = x + Jx, dd = x - Jx each [Ni x Ni] product splits into two [Ni/2 x Ni/2] ones: half the
-//             flops and half the matrix bytes.
-//             Inputs arrive by TMA (one cp.async.bulk.tensor per field and item: box = Ni rows x one member
-//             group, landing directly in the padded panel layout).  A warp owns all rows of its columns, so the
-//             chain needs no CTA barrier and the warps of an SM overlap each other's loads, DMMA sweeps and stores.
-//   k_mean  : mean flow (row a10): U00, W00 of Eq. 14-15 with the wall lift f+-  and the mass-flux
-//             pressure gamma solved so that the discrete bulk flux is held; runs on a side
-//             stream under the per-pair kernel.
+//   k_ypair : one CTA per (kx,kz) pair and member tile.  Everything that couples only along y is chained in
+//             shared memory: F,G assembly (Eq. 4-5), RK3 combination, the precomputed-inverse
+//             solves of Eq. 12-13 for ALL members of the tile at once, dv/dy, the u,w
+//             reconstruction of Eq. 17-18 and du/dy, dw/dy.  The contractions run on the fp64 tensor cores
+//             (DMMA.8x8x4; the only fp64 MMA shape sm_100a executes natively) in the REFLECTION-PARITY basis:
+//             with J the reversal y -> -y of the interior Gauss-Lobatto points, the Chebyshev matrix obeys
+//             J D J = -D and every solve matrix J M J = M, so in the variables s = x + Jx, dd = x - Jx each
+//             [Ni x Ni] product splits into two [Ni/2 x Ni/2] ones: half the flops and half the matrix bytes.
+//             The first CTAs of the grid do the mean flow instead (row a10): U00, W00 of Eq. 14-15 with the wall
+//             lift f+-  and the mass-flux pressure gamma solved so that the discrete bulk flux is
+//             held; they run in the shadow of the pair CTAs.
 // plus layout conversion, input normalisation and diagnostics.
 #include <cuda.h>
 
@@ -57,64 +52,44 @@ __device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* tm, in
                  : "memory");
 }
 
-// One k-sweep of two parity blocks for MTG m-tiles x NT n-tiles at once:
-//   accS[m][nt] += AS[rows 8 (mg0+m)..+7][:] * B_S[:][8 nt..+7],   accD likewise with AD, B_D.
+// One k-sweep of two parity blocks at once (four independent accumulator chains per n-tile pair keep the DMMA
+// pipe busy):  accS[nt] += AS[rows 8 mt..+7][:] * B_S[:][col0 + 8 nt..+7],  accD likewise with AD, B_D.
 // AS, AD are parity blocks in DMMA fragment order (plan.cu: fold_block): a warp reads 512 contiguous bytes per
-// m-tile and pair of k-steps.  The B operands are the warp's own parity panels in shared memory: row k of the s part
-// is smem row k, row k of the dd part is smem row Ni-1-k (REV).  Every B fragment feeds MTG DMMAs and every A
-// fragment NT DMMAs, which is what keeps the shared-memory/L1 pipe below the DMMA pipe.
-template <int NT, int MTG, int KS2T, bool REVS, bool REVD>
-__device__ __forceinline__ void gemm2m(double (&accS)[MTG][NT][2], double (&accD)[MTG][NT][2],
-                                       const double* __restrict__ AS, const double* __restrict__ AD, const double* BS,
-                                       const double* BD, int KS2r, int mg0, int lane, int ld, int Ni) {
+// pair of k-steps.  The B operands are parity panels in shared memory: row k of the s part is smem row k, row k
+// of the dd part is smem row Ni-1-k (REV).
+template <int NT, int KS2T, bool REVS, bool REVD>
+__device__ __forceinline__ void gemm2(double (&accS)[NT][2], double (&accD)[NT][2], const double* __restrict__ AS,
+                                      const double* __restrict__ AD, const double* BS, const double* BD, int KS2r,
+                                      int mt, int lane, int ld, int Ni, int col0) {
     const int KS2 = KS2T ? KS2T : KS2r;
     const int g = lane >> 2, t = lane & 3;
-    const double2* AfS = reinterpret_cast<const double2*>(AS) + lane;
-    const double2* AfD = reinterpret_cast<const double2*>(AD) + lane;
-    const double* BcS = BS + g;
-    const double* BcD = BD + g;
+    const double2* AfS = reinterpret_cast<const double2*>(AS) + (size_t)mt * KS2 * 32 + lane;
+    const double2* AfD = reinterpret_cast<const double2*>(AD) + (size_t)mt * KS2 * 32 + lane;
+    const double* BcS = BS + col0 + g;
+    const double* BcD = BD + col0 + g;
 #pragma unroll
     for (int ks2 = 0; ks2 < KS2; ++ks2) {
-        double2 aS[MTG], aD[MTG];
-#pragma unroll
-        for (int m = 0; m < MTG; ++m) {
-            const int mt = mg0 + m < KS2 ? mg0 + m : KS2 - 1;          // clamped: rows past the end are never stored
-            aS[m] = __ldg(AfS + ((size_t)mt * KS2 + ks2) * 32);
-            aD[m] = __ldg(AfD + ((size_t)mt * KS2 + ks2) * 32);
-        }
+        const double2 aS = __ldg(AfS + ks2 * 32), aD = __ldg(AfD + ks2 * 32);
         const int k = 8 * ks2 + t;
         const int f0 = min(k, Ni - 1), f1 = min(k + 4, Ni - 1), r0 = max(Ni - 1 - k, 0), r1 = max(Ni - 5 - k, 0);
         const double* s0 = BcS + (REVS ? r0 : f0) * ld;
         const double* s1 = BcS + (REVS ? r1 : f1) * ld;
         const double* d0 = BcD + (REVD ? r0 : f0) * ld;
         const double* d1 = BcD + (REVD ? r1 : f1) * ld;
-        double bS0[NT], bS1[NT], bD0[NT], bD1[NT];
 #pragma unroll
-        for (int nt = 0; nt < NT; ++nt) { bS0[nt] = s0[8 * nt]; bD0[nt] = d0[8 * nt]; bS1[nt] = s1[8 * nt]; bD1[nt] = d1[8 * nt]; }
+        for (int nt = 0; nt < NT; ++nt) { dmma(accS[nt], aS.x, s0[8 * nt]); dmma(accD[nt], aD.x, d0[8 * nt]); }
 #pragma unroll
-        for (int m = 0; m < MTG; ++m)
-#pragma unroll
-            for (int nt = 0; nt < NT; ++nt) { dmma(accS[m][nt], aS[m].x, bS0[nt]); dmma(accD[m][nt], aD[m].x, bD0[nt]); }
-#pragma unroll
-        for (int m = 0; m < MTG; ++m)
-#pragma unroll
-            for (int nt = 0; nt < NT; ++nt) { dmma(accS[m][nt], aS[m].y, bS1[nt]); dmma(accD[m][nt], aD[m].y, bD1[nt]); }
+        for (int nt = 0; nt < NT; ++nt) { dmma(accS[nt], aS.y, s1[8 * nt]); dmma(accD[nt], aD.y, d1[8 * nt]); }
     }
 }
 
-template <int NT, int MTG> __device__ __forceinline__ void zero_acc(double (&acc)[MTG][NT][2]) {
+template <int NT> __device__ __forceinline__ void zero_acc(double (&acc)[NT][2]) {
 #pragma unroll
-    for (int m = 0; m < MTG; ++m)
-#pragma unroll
-        for (int nt = 0; nt < NT; ++nt) acc[m][nt][0] = acc[m][nt][1] = 0.0;
+    for (int nt = 0; nt < NT; ++nt) acc[nt][0] = acc[nt][1] = 0.0;
 }
 
 __device__ __forceinline__ double2 ld2(const double* p) { return *reinterpret_cast<const double2*>(p); }
 __device__ __forceinline__ void st2(double* p, double2 v) { *reinterpret_cast<double2*>(p) = v; }
-__device__ __forceinline__ double2 add2(double2 a, double2 b) { return make_double2(a.x + b.x, a.y + b.y); }
-__device__ __forceinline__ double2 sub2(double2 a, double2 b) { return make_double2(a.x - b.x, a.y - b.y); }
-__device__ __forceinline__ double2 hsum2(double2 a, double2 b) { return make_double2(0.5 * (a.x + b.x), 0.5 * (a.y + b.y)); }
-__device__ __forceinline__ double2 hdif2(double2 a, double2 b) { return make_double2(0.5 * (a.x - b.x), 0.5 * (a.y - b.y)); }
 
 // ------------------------------------------------------------------------------------------------ mean flow
 // CTA-wide: tiles of 8 members x (blockDim/8) row slots; dynamic smem = 6 vectors [Ny][8]
@@ -213,326 +188,290 @@ __device__ void mean_body(const DnsDev& d, int stage, int derive_only, int tile,
 }
 
 // ------------------------------------------------------------------------------------------------ per-pair chain
-// Every WARP is an independent worker: it owns 8 NT columns (4 NT members) of one (kx,kz) pair, i.e. all rows of
-// both parities of those columns, so the whole chain F,G -> solves -> dv/dy -> u,w -> du/dy,dw/dy is warp-local
-// (columns never mix): no CTA barrier anywhere, warps drift apart and overlap each other's TMA waits, DMMA sweeps
-// and stores.  Work items (pair, member group) are handed out by an atomic counter.
-// grid = persistent CTAs (one per SM) ; block = 32 * warps-that-fit ; dynamic smem = 5 panels of Ni x ld doubles per warp.
-constexpr int YP_MAXW = 8;
+// grid = nmean + (P-1) * ntile_e ; block = 32 * (Kp/8) * NWN ; dynamic smem = 5 panels of Ni x ld doubles.
+// A warp owns m-tile mt (rows 8 mt..+7 of BOTH parities) and NT n-tiles (members 4 NT wn .. of the tile).
+#ifndef DNS_YP_REGCAP
+#define DNS_YP_REGCAP 128
+#endif
+// CTAs per SM the register allocation is asked to allow: as many as fit with DNS_YP_REGCAP registers per thread
+constexpr int ypair_minb(int threads) {
+    return threads == 0 ? 1 : (65536 / (threads * DNS_YP_REGCAP) > 0 ? 65536 / (threads * DNS_YP_REGCAP) : 1);
+}
 
-template <int NT, int MTG, int KS2T>
-__global__ void __launch_bounds__(32 * YP_MAXW, 1)
+template <int NT, int NWNT, int KS2T>
+__global__ void __launch_bounds__(KS2T ? 32 * KS2T * NWNT : 1024, ypair_minb(32 * KS2T * NWNT))
 k_ypair(DnsDev d, const __grid_constant__ CUtensorMap tmN, const __grid_constant__ CUtensorMap tmV,
-        const __grid_constant__ CUtensorMap tmE, int stage, int derive_only, int nitems) {
+        const __grid_constant__ CUtensorMap tmE, int stage, int derive_only, int nmean) {
     extern __shared__ __align__(128) double smy[];
-    __shared__ uint64_t bars[YP_MAXW];
+    __shared__ uint64_t bar;
+    if ((int)blockIdx.x < nmean) { mean_body(d, stage, derive_only, blockIdx.x, smy); return; }
+    const int bid = blockIdx.x - nmean;
     const int Ni = d.Ni, KS2 = KS2T ? KS2T : (d.Kp >> 3), Kp = 8 * KS2, Kh = (Ni + 1) >> 1, Kho = Ni >> 1;
-    constexpr int NC = 8 * NT, ETW = 4 * NT, ld = NC + 4;
+    constexpr int NWN = NWNT, NC = 8 * NT * NWN, ET = NC >> 1, ld = NC + 4;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
-    const int ntile_e = (d.E + ETW - 1) / ETW;
+    const int mt = warp % KS2, wn = warp / KS2;
+    const int ntile_e = (d.E + ET - 1) / ET;
+    const int p = 1 + bid / ntile_e, e0 = (bid % ntile_e) * ET;
+    const int n = p / d.nkz, mi = p % d.nkz;
+    const int mabs = mi < d.nzh ? mi : d.nkz - mi;
+    const double kx = d.kx[n], kz = d.kz[mi], alpha = kx * kx + kz * kz, ialpha = 1.0 / alpha;
     const int hi = stage == 0 ? 0 : 1;
     const double hdt = (stage == 0 ? 0.5 : 1.0) * d.dt;
     const size_t BB = (size_t)Kp * Kp;
+    const double* mA = d.matsP + (((size_t)hi * d.nkx * d.nzh + (size_t)n * d.nzh + mabs) * 6) * BB;
     const double* Dsd = d.Dfrag;            // dd -> s
     const double* Dds = d.Dfrag + BB;       // s -> dd
     const size_t PS = ((size_t)Ni * ld + 15) & ~(size_t)15;      // panel pitch: a multiple of 128 B (TMA destination)
-    const size_t rowstride = (size_t)d.P * d.E;                  // complex elements between consecutive y rows
-    double2* vout = stage == 2 ? d.vt : d.vs;
-    const uint32_t txbytes = (uint32_t)((derive_only ? 2 : 5) * Ni * ld * 8);
-    double* P0 = smy + (size_t)warp * 5 * PS;
+    double* P0 = smy;
     double* P1 = P0 + PS;
     double* P2 = P1 + PS;
     double* P3 = P2 + PS;
     double* P4 = P3 + PS;
-    uint64_t* bar = &bars[warp];
-    if (lane == 0) {
-        mbar_init(bar, 1);
+    const size_t rowstride = (size_t)d.P * d.E;             // complex elements between consecutive y rows
+    const size_t pbase = (size_t)p * d.E + e0;              // + (row + 1) * rowstride + member
+    double2* vout = stage == 2 ? d.vt : d.vs;
+
+    // ---- stage the inputs: one TMA tile per field (box = Ni rows x ld doubles, landing in the padded panel layout;
+    //      the 4 pad columns of every row are the first two members of the neighbouring tile: never used)
+    const int nvalid = d.E - e0 < ET ? d.E - e0 : ET;
+    if (threadIdx.x == 0) {
+        mbar_init(&bar, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    }
-    __syncwarp();
-
-    for (uint32_t itc = 0;; ++itc) {
-        int cur = 0;
-        if (lane == 0) cur = (int)atomicAdd(d.ypctr, 1u);
-        cur = __shfl_sync(0xffffffffu, cur, 0);
-        if (cur >= nitems) break;
-        const int p = 1 + cur / ntile_e, e0 = (cur % ntile_e) * ETW;
-        if (lane == 0) {
-            // box = Ni rows x ld doubles; the 4 pad columns of a row are the next two members: never used
-            const int c0 = 2 * (p * d.E + e0);
-            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");      // the panels were last written by st.shared
-            mbar_arrive_expect_tx(bar, txbytes);
-            if (derive_only) {
-                tma_load_2d(P0, &tmV, c0, 1, bar);
-                tma_load_2d(P4, &tmE, c0, 1, bar);
-            } else {
-                tma_load_2d(P0, &tmN, c0, 1, bar);                  // (u.grad)u
-                tma_load_2d(P1, &tmN, c0, 2 * d.Ny + 1, bar);      // (u.grad)w
-                tma_load_2d(P2, &tmN, c0, d.Ny + 1, bar);          // (u.grad)v
-                tma_load_2d(P3, &tmV, c0, 1, bar);                 // v_t
-                tma_load_2d(P4, &tmE, c0, 1, bar);                 // eta_t
-            }
-        }
-        const int n = p / d.nkz, mi = p % d.nkz;
-        const int mabs = mi < d.nzh ? mi : d.nkz - mi;
-        const double kx = d.kx[n], kz = d.kz[mi], alpha = kx * kx + kz * kz, ialpha = 1.0 / alpha;
-        const double* mA = d.matsP + (((size_t)hi * d.nkx * d.nzh + (size_t)n * d.nzh + mabs) * 6) * BB;
-        const size_t pbase = (size_t)p * d.E + e0;          // + (row + 1) * rowstride + member
-        const int nvalid = d.E - e0 < ETW ? d.E - e0 : ETW;
-        auto eokf = [&](int nt) { return 4 * nt + t < nvalid; };
-        mbar_wait(bar, itc & 1);
-
-        if (!derive_only) {
-            // ---- A (element-wise, in place): natural rows (ia, J ia) -> parity rows.  H = i kx Nu + i kz Nw -> P0;
-            //      G = i kz Nu - i kx Nw (Eq. 5), RK3 combination, 2 eta_t - h dt Gc -> P1; 2 v_t -> P3.
-            //      Nv (P2) and eta_t (P4) stay in natural rows for the epilogues that consume them.
-            const int nq = Kh * ETW;
-#pragma unroll 2
-            for (int q0 = 0; q0 < nq; q0 += 32) {
-                const int q = q0 + lane, ia = q / ETW, e = q - ia * ETW;
-                if (ia >= Kh) continue;
-                const int ib = Ni - 1 - ia;
-                double* a0 = P0 + ia * ld + 2 * e;
-                double* b0 = P0 + ib * ld + 2 * e;
-                const double2 nuA = ld2(a0), nuB = ld2(b0), nwA = ld2(a0 + PS), nwB = ld2(b0 + PS);
-                const double2 vtA = ld2(a0 + 3 * PS), vtB = ld2(b0 + 3 * PS), etA = ld2(a0 + 4 * PS), etB = ld2(b0 + 4 * PS);
-                const double2 HA = make_double2(-kx * nuA.y - kz * nwA.y, kx * nuA.x + kz * nwA.x);
-                const double2 HB = make_double2(-kx * nuB.y - kz * nwB.y, kx * nuB.x + kz * nwB.x);
-                const double2 GA = make_double2(-kz * nuA.y + kx * nwA.y, kz * nuA.x - kx * nwA.x);
-                const double2 GB = make_double2(-kz * nuB.y + kx * nwB.y, kz * nuB.x - kx * nwB.x);
-                double2 GcA = GA, GcB = GB;
-                const bool eok = e < nvalid;
-                const size_t giA = pbase + (size_t)(ia + 1) * rowstride + e, giB = pbase + (size_t)(ib + 1) * rowstride + e;
-                if (stage == 0) {
-                    if (eok) { d.G0[giA] = GA; d.G0[giB] = GB; }
-                } else {
-                    // history: G0 after stage 0, G0 + 4 G1 after stage 1
-                    double2 hA = make_double2(0.0, 0.0), hB = hA;
-                    if (eok) { hA = d.G0[giA]; hB = d.G0[giB]; }
-                    if (stage == 1) {
-                        GcA = make_double2(2.0 * GA.x - hA.x, 2.0 * GA.y - hA.y);
-                        GcB = make_double2(2.0 * GB.x - hB.x, 2.0 * GB.y - hB.y);
-                        if (eok) {
-                            d.G0[giA] = make_double2(hA.x + 4.0 * GA.x, hA.y + 4.0 * GA.y);
-                            d.G0[giB] = make_double2(hB.x + 4.0 * GB.x, hB.y + 4.0 * GB.y);
-                        }
-                    } else {
-                        GcA = make_double2((hA.x + GA.x) / 6.0, (hA.y + GA.y) / 6.0);
-                        GcB = make_double2((hB.x + GB.x) / 6.0, (hB.y + GB.y) / 6.0);
-                    }
-                }
-                const double2 rA = make_double2(2.0 * etA.x - hdt * GcA.x, 2.0 * etA.y - hdt * GcA.y);
-                const double2 rB = make_double2(2.0 * etB.x - hdt * GcB.x, 2.0 * etB.y - hdt * GcB.y);
-                st2(a0, add2(HA, HB));
-                st2(a0 + PS, add2(rA, rB));
-                st2(a0 + 3 * PS, make_double2(2.0 * (vtA.x + vtB.x), 2.0 * (vtA.y + vtB.y)));
-                if (ib != ia) {
-                    st2(b0, sub2(HA, HB));
-                    st2(b0 + PS, sub2(rA, rB));
-                    st2(b0 + 3 * PS, make_double2(2.0 * (vtA.x - vtB.x), 2.0 * (vtA.y - vtB.y)));
-                }
-            }
-            __syncwarp();
-            // ---- B: F = -alpha Nv - D H (Eq. 4 with Eq. 10's sign), RK3 combination; -h dt Fc (parity) -> P2
-            for (int mg0 = 0; mg0 < KS2; mg0 += MTG) {
-                double accS[MTG][NT][2], accD[MTG][NT][2];
-                zero_acc<NT, MTG>(accS); zero_acc<NT, MTG>(accD);
-                gemm2m<NT, MTG, KS2T, true, false>(accS, accD, Dsd, Dds, P0, P0, KS2, mg0, lane, ld, Ni);
-#pragma unroll
-                for (int m = 0; m < MTG; ++m) {
-                    const int i = 8 * (mg0 + m) + g, Ji = Ni - 1 - i;
-                    if (i >= Kh) continue;
-                    const bool dok = i < Kho;
-#pragma unroll
-                    for (int nt = 0; nt < NT; ++nt) {
-                        double* pa = P2 + i * ld + 8 * nt + 2 * t;
-                        double* pb = P2 + Ji * ld + 8 * nt + 2 * t;
-                        const double2 nvA = ld2(pa), nvB = ld2(pb);
-                        // natural rows: (D H)(i) = (S + D)/2, (D H)(J i) = (S - D)/2
-                        const double2 FA = make_double2(-alpha * nvA.x - 0.5 * (accS[m][nt][0] + accD[m][nt][0]),
-                                                        -alpha * nvA.y - 0.5 * (accS[m][nt][1] + accD[m][nt][1]));
-                        const double2 FB = make_double2(-alpha * nvB.x - 0.5 * (accS[m][nt][0] - accD[m][nt][0]),
-                                                        -alpha * nvB.y - 0.5 * (accS[m][nt][1] - accD[m][nt][1]));
-                        double2 cA = FA, cB = FB;
-                        const bool eok = eokf(nt);
-                        const size_t giA = pbase + (size_t)(i + 1) * rowstride + 4 * nt + t;
-                        const size_t giB = pbase + (size_t)(Ji + 1) * rowstride + 4 * nt + t;
-                        if (stage == 0) {
-                            if (eok) { d.F0[giA] = FA; if (dok) d.F0[giB] = FB; }
-                        } else {
-                            double2 hA = make_double2(0.0, 0.0), hB = hA;
-                            if (eok) { hA = d.F0[giA]; if (dok) hB = d.F0[giB]; }
-                            if (stage == 1) {
-                                cA = make_double2(2.0 * FA.x - hA.x, 2.0 * FA.y - hA.y);
-                                cB = make_double2(2.0 * FB.x - hB.x, 2.0 * FB.y - hB.y);
-                                if (eok) {
-                                    d.F0[giA] = make_double2(hA.x + 4.0 * FA.x, hA.y + 4.0 * FA.y);
-                                    if (dok) d.F0[giB] = make_double2(hB.x + 4.0 * FB.x, hB.y + 4.0 * FB.y);
-                                }
-                            } else {
-                                cA = make_double2((hA.x + FA.x) / 6.0, (hA.y + FA.y) / 6.0);
-                                cB = make_double2((hB.x + FB.x) / 6.0, (hB.y + FB.y) / 6.0);
-                            }
-                        }
-                        if (!dok) cB = cA;                      // middle row of an odd Ni: s = 2 x
-                        st2(pa, make_double2(-hdt * (cA.x + cB.x), -hdt * (cA.y + cB.y)));
-                        if (dok) st2(pb, make_double2(-hdt * (cA.x - cB.x), -hdt * (cA.y - cB.y)));
-                    }
-                }
-            }
-            __syncwarp();
-            // ---- C1: v' = Ainv (2 v_t) + AD (-h dt Fc) - v_t (Eq. 12) -> global, P0 (parity)
-            for (int mg0 = 0; mg0 < KS2; mg0 += MTG) {
-                double accS[MTG][NT][2], accD[MTG][NT][2];
-                zero_acc<NT, MTG>(accS); zero_acc<NT, MTG>(accD);
-                gemm2m<NT, MTG, KS2T, false, true>(accS, accD, mA, mA + BB, P3, P3, KS2, mg0, lane, ld, Ni);
-                gemm2m<NT, MTG, KS2T, false, true>(accS, accD, mA + 2 * BB, mA + 3 * BB, P2, P2, KS2, mg0, lane, ld, Ni);
-#pragma unroll
-                for (int m = 0; m < MTG; ++m) {
-                    const int i = 8 * (mg0 + m) + g, Ji = Ni - 1 - i;
-                    if (i >= Kh) continue;
-                    const bool dok = i < Kho;
-#pragma unroll
-                    for (int nt = 0; nt < NT; ++nt) {
-                        const int c = 8 * nt + 2 * t;
-                        const double2 v2S = ld2(P3 + i * ld + c);
-                        const double2 vS = make_double2(accS[m][nt][0] - 0.5 * v2S.x, accS[m][nt][1] - 0.5 * v2S.y);
-                        double2 vD = make_double2(0.0, 0.0);
-                        st2(P0 + i * ld + c, vS);
-                        if (dok) {
-                            const double2 v2D = ld2(P3 + Ji * ld + c);
-                            vD = make_double2(accD[m][nt][0] - 0.5 * v2D.x, accD[m][nt][1] - 0.5 * v2D.y);
-                            st2(P0 + Ji * ld + c, vD);
-                        }
-                        if (eokf(nt)) {
-                            vout[pbase + (size_t)(i + 1) * rowstride + 4 * nt + t] = hsum2(vS, vD);
-                            if (dok) vout[pbase + (size_t)(Ji + 1) * rowstride + 4 * nt + t] = hdif2(vS, vD);
-                        }
-                    }
-                }
-            }
-            // ---- C2: eta' = Sinv (2 eta_t - h dt Gc) - eta_t (Eq. 13) -> P4 (parity), global at the last stage
-            for (int mg0 = 0; mg0 < KS2; mg0 += MTG) {
-                double accS[MTG][NT][2], accD[MTG][NT][2];
-                zero_acc<NT, MTG>(accS); zero_acc<NT, MTG>(accD);
-                gemm2m<NT, MTG, KS2T, false, true>(accS, accD, mA + 4 * BB, mA + 5 * BB, P1, P1, KS2, mg0, lane, ld, Ni);
-#pragma unroll
-                for (int m = 0; m < MTG; ++m) {
-                    const int i = 8 * (mg0 + m) + g, Ji = Ni - 1 - i;
-                    if (i >= Kh) continue;
-                    const bool dok = i < Kho;
-#pragma unroll
-                    for (int nt = 0; nt < NT; ++nt) {
-                        const int c = 8 * nt + 2 * t;
-                        const double2 etA = ld2(P4 + i * ld + c), etB = ld2(P4 + Ji * ld + c);      // natural rows
-                        const double2 eS = make_double2(accS[m][nt][0] - (etA.x + etB.x), accS[m][nt][1] - (etA.y + etB.y));
-                        double2 eD = make_double2(0.0, 0.0);
-                        if (dok) eD = make_double2(accD[m][nt][0] - (etA.x - etB.x), accD[m][nt][1] - (etA.y - etB.y));
-                        st2(P4 + i * ld + c, eS);
-                        if (dok) st2(P4 + Ji * ld + c, eD);
-                        if (stage == 2 && eokf(nt)) {
-                            d.et[pbase + (size_t)(i + 1) * rowstride + 4 * nt + t] = hsum2(eS, eD);
-                            if (dok) d.et[pbase + (size_t)(Ji + 1) * rowstride + 4 * nt + t] = hdif2(eS, eD);
-                        }
-                    }
-                }
-            }
-            __syncwarp();
+        const int c0 = 2 * (p * d.E + e0);
+        mbar_arrive_expect_tx(&bar, (uint32_t)((derive_only ? 2 : 5) * Ni * ld * 8));
+        if (derive_only) {
+            tma_load_2d(P0, &tmV, c0, 1, &bar);
+            tma_load_2d(P4, &tmE, c0, 1, &bar);
         } else {
-            // parity transform of v_t (P0) and eta_t (P4) in place
-            const int nq = Kh * ETW;
-            for (int q0 = 0; q0 < nq; q0 += 32) {
-                const int q = q0 + lane, ia = q / ETW, e = q - ia * ETW;
-                if (ia >= Kh) continue;
-                const int ib = Ni - 1 - ia;
-                double* a0 = P0 + ia * ld + 2 * e;
-                double* b0 = P0 + ib * ld + 2 * e;
-                const double2 vA = ld2(a0), vB = ld2(b0), eA = ld2(a0 + 4 * PS), eB = ld2(b0 + 4 * PS);
-                st2(a0, add2(vA, vB));
-                st2(a0 + 4 * PS, add2(eA, eB));
-                if (ib != ia) {
-                    st2(b0, sub2(vA, vB));
-                    st2(b0 + 4 * PS, sub2(eA, eB));
-                }
-            }
-            __syncwarp();
+            tma_load_2d(P0, &tmN, c0, 1, &bar);                  // (u.grad)u
+            tma_load_2d(P1, &tmN, c0, 2 * d.Ny + 1, &bar);      // (u.grad)w
+            tma_load_2d(P2, &tmN, c0, d.Ny + 1, &bar);          // (u.grad)v
+            tma_load_2d(P3, &tmV, c0, 1, &bar);                 // v_t
+            tma_load_2d(P4, &tmE, c0, 1, &bar);                 // eta_t
         }
-        // ---- D: dv/dy = D v' ; u = (i kx Dv - i kz eta)/alpha, w = (i kz Dv + i kx eta)/alpha (Eq. 17-18) -> global, P2, P3
-        for (int mg0 = 0; mg0 < KS2; mg0 += MTG) {
-            double accS[MTG][NT][2], accD[MTG][NT][2];
-            zero_acc<NT, MTG>(accS); zero_acc<NT, MTG>(accD);
-            gemm2m<NT, MTG, KS2T, true, false>(accS, accD, Dsd, Dds, P0, P0, KS2, mg0, lane, ld, Ni);
-#pragma unroll
-            for (int m = 0; m < MTG; ++m) {
-                const int i = 8 * (mg0 + m) + g, Ji = Ni - 1 - i;
-                if (i >= Kh) continue;
-                const bool dok = i < Kho;
-#pragma unroll
-                for (int nt = 0; nt < NT; ++nt) {
-                    const int c = 8 * nt + 2 * t;
-                    const double2 eS = ld2(P4 + i * ld + c);
-                    const double2 uS = make_double2((-kx * accS[m][nt][1] + kz * eS.y) * ialpha, (kx * accS[m][nt][0] - kz * eS.x) * ialpha);
-                    const double2 wS = make_double2((-kz * accS[m][nt][1] - kx * eS.y) * ialpha, (kz * accS[m][nt][0] + kx * eS.x) * ialpha);
-                    double2 uD = make_double2(0.0, 0.0), wD = uD;
-                    st2(P2 + i * ld + c, uS);
-                    st2(P3 + i * ld + c, wS);
-                    if (dok) {
-                        const double2 eD = ld2(P4 + Ji * ld + c);
-                        uD = make_double2((-kx * accD[m][nt][1] + kz * eD.y) * ialpha, (kx * accD[m][nt][0] - kz * eD.x) * ialpha);
-                        wD = make_double2((-kz * accD[m][nt][1] - kx * eD.y) * ialpha, (kz * accD[m][nt][0] + kx * eD.x) * ialpha);
-                        st2(P2 + Ji * ld + c, uD);
-                        st2(P3 + Ji * ld + c, wD);
-                    }
-                    if (eokf(nt)) {
-                        const size_t giA = pbase + (size_t)(i + 1) * rowstride + 4 * nt + t;
-                        const size_t giB = pbase + (size_t)(Ji + 1) * rowstride + 4 * nt + t;
-                        d.uh[giA] = hsum2(uS, uD);
-                        d.wh[giA] = hsum2(wS, wD);
-                        if (dok) { d.uh[giB] = hdif2(uS, uD); d.wh[giB] = hdif2(wS, wD); }
-                    }
-                }
-            }
-        }
-        __syncwarp();
-        // ---- E: du/dy, dw/dy -> global
-#pragma unroll 1
-        for (int f = 0; f < 2; ++f) {
-            const double* Pin = f == 0 ? P2 : P3;
-            double2* dst = f == 0 ? d.duh : d.dwh;
-            for (int mg0 = 0; mg0 < KS2; mg0 += MTG) {
-                double accS[MTG][NT][2], accD[MTG][NT][2];
-                zero_acc<NT, MTG>(accS); zero_acc<NT, MTG>(accD);
-                gemm2m<NT, MTG, KS2T, true, false>(accS, accD, Dsd, Dds, Pin, Pin, KS2, mg0, lane, ld, Ni);
-#pragma unroll
-                for (int m = 0; m < MTG; ++m) {
-                    const int i = 8 * (mg0 + m) + g, Ji = Ni - 1 - i;
-                    if (i >= Kh) continue;
-#pragma unroll
-                    for (int nt = 0; nt < NT; ++nt) {
-                        if (!eokf(nt)) continue;
-                        dst[pbase + (size_t)(i + 1) * rowstride + 4 * nt + t] =
-                            make_double2(0.5 * (accS[m][nt][0] + accD[m][nt][0]), 0.5 * (accS[m][nt][1] + accD[m][nt][1]));
-                        if (i < Kho)
-                            dst[pbase + (size_t)(Ji + 1) * rowstride + 4 * nt + t] =
-                                make_double2(0.5 * (accS[m][nt][0] - accD[m][nt][0]), 0.5 * (accS[m][nt][1] - accD[m][nt][1]));
-                    }
-                }
-            }
-        }
-        __syncwarp();                                            // all lanes are done with the panels
     }
-    // the last warp to leave re-arms the work counter for the next launch (launches are stream-ordered)
-    if (lane == 0) {
-        __threadfence();
-        const unsigned done = atomicAdd(d.ypctr + 1, 1u);
-        if (done == gridDim.x * (blockDim.x >> 5) - 1) { d.ypctr[0] = 0u; d.ypctr[1] = 0u; __threadfence(); }
-    }
-}
+    __syncthreads();                                         // the barrier is initialised before anyone waits on it
 
-// mean flow as its own small launch (8 members per CTA); api.cu runs it on a side stream under the per-pair kernel
-__global__ void __launch_bounds__(256) k_mean(DnsDev d, int stage, int derive_only) {
-    extern __shared__ __align__(128) double smm[];
-    mean_body(d, stage, derive_only, blockIdx.x, smm);
+    // ---- own fragment elements: row i = 8 mt + g of both parities, columns col0 + 8 nt + 2t, +1 (one member)
+    const int i = 8 * mt + g, Ji = Ni - 1 - i;
+    const bool sok = i < Kh, dok = i < Kho;
+    const int col0 = 8 * NT * wn;
+    const int offS = (sok ? i : 0) * ld + col0 + 2 * t, offD = (dok ? Ji : 0) * ld + col0 + 2 * t;
+    auto eokf = [&](int nt) { return (e0 + (col0 >> 1) + 4 * nt + t) < d.E; };
+    const size_t gS = pbase + (size_t)(i + 1) * rowstride + (col0 >> 1) + t;      // + 4 nt : natural row i
+    const size_t gD = pbase + (size_t)(Ji + 1) * rowstride + (col0 >> 1) + t;     // natural row J i
+
+    // ---- history of the nonlinear terms: hist = N0 after stage 0, N0 + 4 N1 after stage 1
+    double2 fhS[NT], fhD[NT], ghA[NT], ghB[NT];
+    if (!derive_only && stage > 0) {
+#pragma unroll
+        for (int nt = 0; nt < NT; ++nt) {
+            fhS[nt] = fhD[nt] = make_double2(0.0, 0.0);
+            if (eokf(nt)) {
+                if (sok) fhS[nt] = d.F0[gS + 4 * nt];
+                if (dok) fhD[nt] = d.F0[gD + 4 * nt];
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < NT; ++k) {
+            const int q = threadIdx.x + k * blockDim.x, ia = q / ET, e = q - ia * ET;
+            ghA[k] = ghB[k] = make_double2(0.0, 0.0);
+            if (ia < Kh && e < nvalid) {
+                ghA[k] = d.G0[pbase + (size_t)(ia + 1) * rowstride + e];
+                ghB[k] = d.G0[pbase + (size_t)(Ni - ia) * rowstride + e];
+            }
+        }
+    }
+    mbar_wait(&bar, 0);
+
+    double accS[NT][2], accD[NT][2];
+    if (!derive_only) {
+        // ---- A (element-wise, in place): natural rows (ia, J ia) -> parity rows; H = i kx Nu + i kz Nw -> P0,
+        //      G = i kz Nu - i kx Nw (Eq. 5), RK3 combination, 2 eta_t - h dt Gc -> P1, Nv -> P2, 2 v_t -> P3, eta_t -> P4
+#pragma unroll
+        for (int k = 0; k < NT; ++k) {
+            const int q = threadIdx.x + k * blockDim.x, ia = q / ET, e = q - ia * ET;
+            if (ia >= Kh) continue;
+            const int ib = Ni - 1 - ia;
+            double* a0 = P0 + ia * ld + 2 * e;
+            double* b0 = P0 + ib * ld + 2 * e;
+            const double2 nuA = ld2(a0), nuB = ld2(b0), nwA = ld2(a0 + PS), nwB = ld2(b0 + PS);
+            const double2 nvA = ld2(a0 + 2 * PS), nvB = ld2(b0 + 2 * PS), vtA = ld2(a0 + 3 * PS), vtB = ld2(b0 + 3 * PS);
+            const double2 etA = ld2(a0 + 4 * PS), etB = ld2(b0 + 4 * PS);
+            const double2 HA = make_double2(-kx * nuA.y - kz * nwA.y, kx * nuA.x + kz * nwA.x);
+            const double2 HB = make_double2(-kx * nuB.y - kz * nwB.y, kx * nuB.x + kz * nwB.x);
+            const double2 GA = make_double2(-kz * nuA.y + kx * nwA.y, kz * nuA.x - kx * nwA.x);
+            const double2 GB = make_double2(-kz * nuB.y + kx * nwB.y, kz * nuB.x - kx * nwB.x);
+            double2 GcA, GcB;
+            const bool eok = e < nvalid;
+            const size_t giA = pbase + (size_t)(ia + 1) * rowstride + e, giB = pbase + (size_t)(ib + 1) * rowstride + e;
+            if (stage == 0) {
+                GcA = GA; GcB = GB;
+                if (eok) { d.G0[giA] = GA; d.G0[giB] = GB; }
+            } else if (stage == 1) {
+                GcA = make_double2(2.0 * GA.x - ghA[k].x, 2.0 * GA.y - ghA[k].y);
+                GcB = make_double2(2.0 * GB.x - ghB[k].x, 2.0 * GB.y - ghB[k].y);
+                if (eok) {
+                    d.G0[giA] = make_double2(ghA[k].x + 4.0 * GA.x, ghA[k].y + 4.0 * GA.y);
+                    d.G0[giB] = make_double2(ghB[k].x + 4.0 * GB.x, ghB[k].y + 4.0 * GB.y);
+                }
+            } else {
+                GcA = make_double2((ghA[k].x + GA.x) / 6.0, (ghA[k].y + GA.y) / 6.0);
+                GcB = make_double2((ghB[k].x + GB.x) / 6.0, (ghB[k].y + GB.y) / 6.0);
+            }
+            const double2 rA = make_double2(2.0 * etA.x - hdt * GcA.x, 2.0 * etA.y - hdt * GcA.y);
+            const double2 rB = make_double2(2.0 * etB.x - hdt * GcB.x, 2.0 * etB.y - hdt * GcB.y);
+            st2(a0, make_double2(HA.x + HB.x, HA.y + HB.y));
+            st2(a0 + PS, make_double2(rA.x + rB.x, rA.y + rB.y));
+            st2(a0 + 2 * PS, make_double2(nvA.x + nvB.x, nvA.y + nvB.y));
+            st2(a0 + 3 * PS, make_double2(2.0 * (vtA.x + vtB.x), 2.0 * (vtA.y + vtB.y)));
+            st2(a0 + 4 * PS, make_double2(etA.x + etB.x, etA.y + etB.y));
+            if (ib != ia) {
+                st2(b0, make_double2(HA.x - HB.x, HA.y - HB.y));
+                st2(b0 + PS, make_double2(rA.x - rB.x, rA.y - rB.y));
+                st2(b0 + 2 * PS, make_double2(nvA.x - nvB.x, nvA.y - nvB.y));
+                st2(b0 + 3 * PS, make_double2(2.0 * (vtA.x - vtB.x), 2.0 * (vtA.y - vtB.y)));
+                st2(b0 + 4 * PS, make_double2(etA.x - etB.x, etA.y - etB.y));
+            }
+        }
+        __syncthreads();
+        // ---- B: F = -alpha Nv - D H (Eq. 4 with Eq. 10's sign), RK3 combination; -h dt Fc -> P2
+        zero_acc<NT>(accS); zero_acc<NT>(accD);
+        gemm2<NT, KS2T, true, false>(accS, accD, Dsd, Dds, P0, P0, KS2, mt, lane, ld, Ni, col0);
+#pragma unroll
+        for (int nt = 0; nt < NT; ++nt) {
+            double2 FS = make_double2(0.0, 0.0), FD = make_double2(0.0, 0.0);
+            if (sok) { const double2 nv = ld2(P2 + offS + 8 * nt); FS = make_double2(-alpha * nv.x - accS[nt][0], -alpha * nv.y - accS[nt][1]); }
+            if (dok) { const double2 nv = ld2(P2 + offD + 8 * nt); FD = make_double2(-alpha * nv.x - accD[nt][0], -alpha * nv.y - accD[nt][1]); }
+            // natural rows: F(i) = (FS + FD)/2, F(Ji) = (FS - FD)/2
+            const double2 FA = make_double2(0.5 * (FS.x + FD.x), 0.5 * (FS.y + FD.y));
+            const double2 FB = make_double2(0.5 * (FS.x - FD.x), 0.5 * (FS.y - FD.y));
+            double2 cA, cB;
+            const bool eok = eokf(nt);
+            if (stage == 0) {
+                cA = FA; cB = FB;
+                if (eok && sok) d.F0[gS + 4 * nt] = FA;
+                if (eok && dok) d.F0[gD + 4 * nt] = FB;
+            } else if (stage == 1) {
+                cA = make_double2(2.0 * FA.x - fhS[nt].x, 2.0 * FA.y - fhS[nt].y);
+                cB = make_double2(2.0 * FB.x - fhD[nt].x, 2.0 * FB.y - fhD[nt].y);
+                if (eok && sok) d.F0[gS + 4 * nt] = make_double2(fhS[nt].x + 4.0 * FA.x, fhS[nt].y + 4.0 * FA.y);
+                if (eok && dok) d.F0[gD + 4 * nt] = make_double2(fhD[nt].x + 4.0 * FB.x, fhD[nt].y + 4.0 * FB.y);
+            } else {
+                cA = make_double2((fhS[nt].x + FA.x) / 6.0, (fhS[nt].y + FA.y) / 6.0);
+                cB = make_double2((fhD[nt].x + FB.x) / 6.0, (fhD[nt].y + FB.y) / 6.0);
+            }
+            if (!dok) cB = cA;                              // middle row of an odd Ni: s = 2 x
+            if (sok) st2(P2 + offS + 8 * nt, make_double2(-hdt * (cA.x + cB.x), -hdt * (cA.y + cB.y)));
+            if (dok) st2(P2 + offD + 8 * nt, make_double2(-hdt * (cA.x - cB.x), -hdt * (cA.y - cB.y)));
+        }
+        __syncthreads();
+        // ---- C: v' = Ainv (2 v_t) + AD (-h dt Fc) - v_t (Eq. 12) -> global, P0 ; eta' = Sinv P1 - eta_t (Eq. 13) -> P4
+        zero_acc<NT>(accS); zero_acc<NT>(accD);
+        gemm2<NT, KS2T, false, true>(accS, accD, mA, mA + BB, P3, P3, KS2, mt, lane, ld, Ni, col0);
+        gemm2<NT, KS2T, false, true>(accS, accD, mA + 2 * BB, mA + 3 * BB, P2, P2, KS2, mt, lane, ld, Ni, col0);
+        double acc2S[NT][2], acc2D[NT][2];
+        zero_acc<NT>(acc2S); zero_acc<NT>(acc2D);
+        gemm2<NT, KS2T, false, true>(acc2S, acc2D, mA + 4 * BB, mA + 5 * BB, P1, P1, KS2, mt, lane, ld, Ni, col0);
+#pragma unroll
+        for (int nt = 0; nt < NT; ++nt) {
+            double2 vS = make_double2(0.0, 0.0), vD = vS, eS = vS, eD = vS;
+            if (sok) {
+                const double2 v2 = ld2(P3 + offS + 8 * nt), et = ld2(P4 + offS + 8 * nt);
+                vS = make_double2(accS[nt][0] - 0.5 * v2.x, accS[nt][1] - 0.5 * v2.y);
+                eS = make_double2(acc2S[nt][0] - et.x, acc2S[nt][1] - et.y);
+                st2(P0 + offS + 8 * nt, vS);
+                st2(P4 + offS + 8 * nt, eS);
+            }
+            if (dok) {
+                const double2 v2 = ld2(P3 + offD + 8 * nt), et = ld2(P4 + offD + 8 * nt);
+                vD = make_double2(accD[nt][0] - 0.5 * v2.x, accD[nt][1] - 0.5 * v2.y);
+                eD = make_double2(acc2D[nt][0] - et.x, acc2D[nt][1] - et.y);
+                st2(P0 + offD + 8 * nt, vD);
+                st2(P4 + offD + 8 * nt, eD);
+            }
+            if (eokf(nt)) {
+                if (sok) {
+                    vout[gS + 4 * nt] = make_double2(0.5 * (vS.x + vD.x), 0.5 * (vS.y + vD.y));
+                    if (stage == 2) d.et[gS + 4 * nt] = make_double2(0.5 * (eS.x + eD.x), 0.5 * (eS.y + eD.y));
+                }
+                if (dok) {
+                    vout[gD + 4 * nt] = make_double2(0.5 * (vS.x - vD.x), 0.5 * (vS.y - vD.y));
+                    if (stage == 2) d.et[gD + 4 * nt] = make_double2(0.5 * (eS.x - eD.x), 0.5 * (eS.y - eD.y));
+                }
+            }
+        }
+        __syncthreads();
+    } else {
+        // parity transform of v_t (P0) and eta_t (P4) in place
+#pragma unroll
+        for (int k = 0; k < NT; ++k) {
+            const int q = threadIdx.x + k * blockDim.x, ia = q / ET, e = q - ia * ET;
+            if (ia >= Kh) continue;
+            const int ib = Ni - 1 - ia;
+            double* a0 = P0 + ia * ld + 2 * e;
+            double* b0 = P0 + ib * ld + 2 * e;
+            const double2 vA = ld2(a0), vB = ld2(b0), eA = ld2(a0 + 4 * PS), eB = ld2(b0 + 4 * PS);
+            st2(a0, make_double2(vA.x + vB.x, vA.y + vB.y));
+            st2(a0 + 4 * PS, make_double2(eA.x + eB.x, eA.y + eB.y));
+            if (ib != ia) {
+                st2(b0, make_double2(vA.x - vB.x, vA.y - vB.y));
+                st2(b0 + 4 * PS, make_double2(eA.x - eB.x, eA.y - eB.y));
+            }
+        }
+        __syncthreads();
+    }
+    // ---- D: dv/dy = D v' ; u = (i kx Dv - i kz eta)/alpha, w = (i kz Dv + i kx eta)/alpha (Eq. 17-18) -> global, P2, P3
+    zero_acc<NT>(accS); zero_acc<NT>(accD);
+    gemm2<NT, KS2T, true, false>(accS, accD, Dsd, Dds, P0, P0, KS2, mt, lane, ld, Ni, col0);
+#pragma unroll
+    for (int nt = 0; nt < NT; ++nt) {
+        double2 uS = make_double2(0.0, 0.0), uD = uS, wS = uS, wD = uS;
+        if (sok) {
+            const double2 en = ld2(P4 + offS + 8 * nt);
+            uS = make_double2((-kx * accS[nt][1] + kz * en.y) * ialpha, (kx * accS[nt][0] - kz * en.x) * ialpha);
+            wS = make_double2((-kz * accS[nt][1] - kx * en.y) * ialpha, (kz * accS[nt][0] + kx * en.x) * ialpha);
+            st2(P2 + offS + 8 * nt, uS);
+            st2(P3 + offS + 8 * nt, wS);
+        }
+        if (dok) {
+            const double2 en = ld2(P4 + offD + 8 * nt);
+            uD = make_double2((-kx * accD[nt][1] + kz * en.y) * ialpha, (kx * accD[nt][0] - kz * en.x) * ialpha);
+            wD = make_double2((-kz * accD[nt][1] - kx * en.y) * ialpha, (kz * accD[nt][0] + kx * en.x) * ialpha);
+            st2(P2 + offD + 8 * nt, uD);
+            st2(P3 + offD + 8 * nt, wD);
+        }
+        if (eokf(nt)) {
+            if (sok) {
+                d.uh[gS + 4 * nt] = make_double2(0.5 * (uS.x + uD.x), 0.5 * (uS.y + uD.y));
+                d.wh[gS + 4 * nt] = make_double2(0.5 * (wS.x + wD.x), 0.5 * (wS.y + wD.y));
+            }
+            if (dok) {
+                d.uh[gD + 4 * nt] = make_double2(0.5 * (uS.x - uD.x), 0.5 * (uS.y - uD.y));
+                d.wh[gD + 4 * nt] = make_double2(0.5 * (wS.x - wD.x), 0.5 * (wS.y - wD.y));
+            }
+        }
+    }
+    __syncthreads();
+    // ---- E: du/dy, dw/dy
+    {
+        double a2S[NT][2], a2D[NT][2];
+        zero_acc<NT>(accS); zero_acc<NT>(accD); zero_acc<NT>(a2S); zero_acc<NT>(a2D);
+        gemm2<NT, KS2T, true, false>(accS, accD, Dsd, Dds, P2, P2, KS2, mt, lane, ld, Ni, col0);
+        gemm2<NT, KS2T, true, false>(a2S, a2D, Dsd, Dds, P3, P3, KS2, mt, lane, ld, Ni, col0);
+#pragma unroll
+        for (int nt = 0; nt < NT; ++nt) {
+            if (!eokf(nt)) continue;
+            if (sok) {
+                d.duh[gS + 4 * nt] = make_double2(0.5 * (accS[nt][0] + accD[nt][0]), 0.5 * (accS[nt][1] + accD[nt][1]));
+                d.dwh[gS + 4 * nt] = make_double2(0.5 * (a2S[nt][0] + a2D[nt][0]), 0.5 * (a2S[nt][1] + a2D[nt][1]));
+            }
+            if (dok) {
+                d.duh[gD + 4 * nt] = make_double2(0.5 * (accS[nt][0] - accD[nt][0]), 0.5 * (accS[nt][1] - accD[nt][1]));
+                d.dwh[gD + 4 * nt] = make_double2(0.5 * (a2S[nt][0] - a2D[nt][0]), 0.5 * (a2S[nt][1] - a2D[nt][1]));
+            }
+        }
+    }
 }
 
 // ------------------------------------------------------------------------------------------------ layout / IO
@@ -639,13 +578,13 @@ __global__ void k_diag_rows(DnsDev d, const double* __restrict__ part, double t)
 
 }  // namespace
 
-// bytes of shared memory one warp of the per-pair kernel needs (5 panels of Ni x (8 NT + 4) doubles, 128 B pitch)
-size_t dns_ypair_smem(int Ni, int NT) {
-    return 5 * ((((size_t)Ni * (8 * NT + 4) + 15) & ~(size_t)15) * sizeof(double));
+size_t dns_ypair_smem(int Ni, int Ny, int ET) {
+    const size_t panels = 5 * ((((size_t)Ni * (2 * ET + 4) + 15) & ~(size_t)15) * sizeof(double)), mean = (size_t)6 * Ny * 8 * sizeof(double);
+    return panels > mean ? panels : mean;
 }
 
 // TMA descriptors of the per-pair kernel's inputs: 2-D views [rows][2 P E doubles] of the spectral arrays with a
-// box of Ni rows x (8 NT + 4) doubles, i.e. exactly one padded shared-memory panel.  Encoded at dns_plan_bind.
+// box of Ni rows x (2 ET + 4) doubles, i.e. exactly one padded shared-memory panel.  Encoded at dns_plan_bind.
 int dns_ypair_encode_maps(dns_plan* p) {
     typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                   const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
@@ -663,7 +602,7 @@ int dns_ypair_encode_maps(dns_plan* p) {
     for (int i = 0; i < 3; ++i) {
         const cuuint64_t dims[2] = {(cuuint64_t)2 * d.P * d.E, src[i].rows};
         const cuuint64_t strides[1] = {(cuuint64_t)d.P * d.E * sizeof(double2)};
-        const cuuint32_t box[2] = {(cuuint32_t)(8 * p->NTy + 4), (cuuint32_t)d.Ni};
+        const cuuint32_t box[2] = {(cuuint32_t)(2 * p->ETy + 4), (cuuint32_t)d.Ni};
         const cuuint32_t estr[2] = {1, 1};
         CUresult r = encode(reinterpret_cast<CUtensorMap*>(&p->tmaps[i]), CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, src[i].ptr, dims,
                             strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
@@ -673,56 +612,38 @@ int dns_ypair_encode_maps(dns_plan* p) {
     return DNS_OK;
 }
 
-template <int NT, int MTG, int K> static void ypair_launch_k(dns_plan* p, int stage, int derive_only) {
+template <int NT, int NWN> static void ypair_launch(dns_plan* p, int stage, int derive_only) {
     const DnsDev& d = p->d;
-    const int nitems = (d.P - 1) * ((d.E + 4 * NT - 1) / (4 * NT));
-    const size_t per_warp = dns_ypair_smem(d.Ni, NT);
-    auto kern = k_ypair<NT, MTG, K>;
-    if (p->ypair_grid == 0) {
-        int nsm = 0, dev = 0;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
-        int nw = (int)((226 * 1024) / per_warp);                  // warps whose panels fit one SM
-        if (nw > YP_MAXW) nw = YP_MAXW;
-        if (nw < 1) nw = 1;
-        if (const char* s = getenv("DNS_YP_WARPS")) { int v = atoi(s); if (v >= 1 && v <= nw) nw = v; }
-        const int need = (nitems + nsm - 1) / nsm;                // few items: spread them over all SMs
-        if (nw > need) nw = need < 1 ? 1 : need;
-        p->ypair_warps = nw;
-        p->ypair_grid = nsm;
-        cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(nw * per_warp));
-        cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    const int KS2 = d.Kp >> 3, ET = 4 * NT * NWN;
+    const int nmean = (d.E + 7) / 8;
+    const unsigned grid = (unsigned)(nmean + (d.P - 1) * ((d.E + ET - 1) / ET));
+    const size_t smem = dns_ypair_smem(d.Ni, d.Ny, ET);
+#define LAUNCH(K)                                                                                     \
+    {                                                                                                 \
+        auto kern = k_ypair<NT, NWN, K>;                                                              \
+        cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);           \
+        cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared); \
+        const CUtensorMap* tm = reinterpret_cast<const CUtensorMap*>(p->tmaps);                       \
+        kern<<<grid, 32 * KS2 * NWN, smem, p->stream>>>(d, tm[0], tm[1], tm[2], stage, derive_only, nmean); \
     }
-    const int nw = p->ypair_warps;
-    int grid = (nitems + nw - 1) / nw;
-    if (grid > p->ypair_grid) grid = p->ypair_grid;
-    const CUtensorMap* tm = reinterpret_cast<const CUtensorMap*>(p->tmaps);
-    kern<<<grid, 32 * nw, nw * per_warp, p->stream>>>(d, tm[0], tm[1], tm[2], stage, derive_only, nitems);
-}
-
-template <int NT> static void ypair_launch(dns_plan* p, int stage, int derive_only) {
-    const int KS2 = p->d.Kp >> 3;
     switch (KS2) {
-        case 2: ypair_launch_k<NT, 2, 2>(p, stage, derive_only); break;
-        case 3: ypair_launch_k<NT, 3, 3>(p, stage, derive_only); break;
-        case 4: ypair_launch_k<NT, 4, 4>(p, stage, derive_only); break;
-        case 6: ypair_launch_k<NT, 3, 6>(p, stage, derive_only); break;
-        default:
-            if (KS2 % 2 == 0) ypair_launch_k<NT, 2, 0>(p, stage, derive_only);
-            else ypair_launch_k<NT, 1, 0>(p, stage, derive_only);
-            break;
+        case 2: LAUNCH(2) break;
+        case 3: LAUNCH(3) break;
+        case 4: LAUNCH(4) break;
+        case 6: LAUNCH(6) break;
+        default: LAUNCH(0) break;
     }
+#undef LAUNCH
 }
 
 void launch_ypair(dns_plan* p, int stage, int derive_only) {
-    if (p->NTy == 1) ypair_launch<1>(p, stage, derive_only);
-    else ypair_launch<2>(p, stage, derive_only);
-}
-
-void launch_mean(dns_plan* p, int stage, int derive_only, cudaStream_t stream) {
-    const DnsDev& d = p->d;
-    const size_t smem = (size_t)6 * d.Ny * 8 * sizeof(double);
-    k_mean<<<(d.E + 7) / 8, 256, smem, stream>>>(d, stage, derive_only);
+    const int NT = p->NTy, NWN = p->ETy / (4 * NT);
+    if (NT == 1 && NWN == 1) ypair_launch<1, 1>(p, stage, derive_only);
+    else if (NT == 2 && NWN == 1) ypair_launch<2, 1>(p, stage, derive_only);
+    else if (NT == 1 && NWN == 2) ypair_launch<1, 2>(p, stage, derive_only);
+    else if (NT == 2 && NWN == 2) ypair_launch<2, 2>(p, stage, derive_only);
+    else if (NT == 4 && NWN == 1) ypair_launch<4, 1>(p, stage, derive_only);
+    else ypair_launch<1, 4>(p, stage, derive_only);
 }
 
 void launch_abi_to_internal(dns_plan* p, const double2* src, double2* dst) {
