@@ -116,7 +116,8 @@ int dns_plan_create(dns_plan** out, int Nx, int Ny, int Nz, int E, double Re, do
     d.dt = dt; d.Re = Re; d.Uw = flow == DNS_COUETTE ? 1.0 : 0.0; d.invMxMz = 1.0 / ((double)Mx * Mz);
     d.S = (size_t)Ny * d.P * E;
     {
-        const int tps = dns_line_tps(Mx);                // lanes per slot of the line kernel = largest member tile
+        const int tps = dns_line_tps(Mx, E);             // lanes per slot of the line kernel = largest member tile
+        p->line_tps = tps;
         int et = 1, lg = 0;
         while (et < tps && et < E) { et <<= 1; ++lg; }
         d.etl = lg;
@@ -126,6 +127,7 @@ int dns_plan_create(dns_plan** out, int Nx, int Ny, int Nz, int E, double Re, do
     p->Lx = Lx; p->Lz = Lz;
     // member tiles
     p->ETf = pow2ceil(E) < 32 ? pow2ceil(E) : 32;
+    if (const char* s = getenv("DNS_ETF")) { int v = atoi(s); if ((v == 4 || v == 8 || v == 16 || v == 32) && v <= pow2ceil(E)) p->ETf = v; }
     d.Kp = (((d.Ni + 1) / 2 + 7) / 8) * 8;
     int ETy = pow2ceil(E) < 16 ? pow2ceil(E) : 16;
     if (ETy < 4) ETy = 4;

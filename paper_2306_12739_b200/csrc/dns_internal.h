@@ -59,6 +59,7 @@ struct dns_plan {
     int ETy = 0, NTy = 0;                      // member tile of the per-pair kernel, n-tiles per warp
     int ETf = 0;                               // member tile of the transform kernels
     int line_grid = 0;                         // persistent grid of the line kernel (set at first launch)
+    int line_tps = 0;                          // lanes per slot of the line kernel (4, 8 or 16)
     alignas(64) unsigned char tmaps[3][128];   // CUtensorMap of Nh, vt, et (encoded at dns_plan_bind)
     std::vector<void*> owned;                  // plan-owned device allocations
     void* workspace = nullptr;
@@ -74,7 +75,7 @@ struct dns_plan {
 // host precompute (plan.cu)
 int dns_host_precompute(dns_plan* p);
 bool dns_factor_len(int M, int* R1, int* R2);
-int dns_line_tps(int Mx);
+int dns_line_tps(int Mx, int E);
 
 // kernel launchers (kernels_*.cu); stage = 0,1,2
 void launch_zinv(dns_plan* p, const double2* vin);

@@ -26,8 +26,11 @@ __device__ __forceinline__ int pos_to_mi(int pos, int M, int nzh, int nkz) {
 
 // ------------------------------------------------------------------------------------------------ z inverse
 // grid.x = Ni * nblk_n * ntile_e, grid.y = 5 input fields (u, v, w, Du, Dw); block = 256
+#ifndef DNS_FFT_MINB
+#define DNS_FFT_MINB 2
+#endif
 template <int R1, int R2>
-__global__ void __launch_bounds__(256) k_zinv(DnsDev d, const double2* __restrict__ vin, int etlog, int NB) {
+__global__ void __launch_bounds__(256, DNS_FFT_MINB) k_zinv(DnsDev d, const double2* __restrict__ vin, int etlog, int NB) {
     constexpr int M = R1 * R2;
     extern __shared__ double2 sm[];
     const int ET = 1 << etlog, e_l = threadIdx.x & (ET - 1), slot = threadIdx.x >> etlog, nslots = blockDim.x >> etlog;
