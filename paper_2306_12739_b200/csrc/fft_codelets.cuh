@@ -33,6 +33,9 @@ DNS_DEF_TW(8)
 DNS_DEF_TW(9)
 DNS_DEF_TW(12)
 DNS_DEF_TW(16)
+DNS_DEF_TW(18)
+DNS_DEF_TW(24)
+DNS_DEF_TW(36)
 template <> struct TW<6> {
     DNS_HD static constexpr double c(int k) { return TW<12>::c(2 * k); }
     DNS_HD static constexpr double s(int k) { return TW<12>::s(2 * k); }
@@ -111,5 +114,9 @@ template <> struct DFT<8> { DNS_HD static void run(double2 (&x)[8]) { dft_ct<2, 
 template <> struct DFT<9> { DNS_HD static void run(double2 (&x)[9]) { dft_ct<3, 3>(x); } };
 template <> struct DFT<12> { DNS_HD static void run(double2 (&x)[12]) { dft_ct<3, 4>(x); } };
 template <> struct DFT<16> { DNS_HD static void run(double2 (&x)[16]) { dft_ct<4, 4>(x); } };
+// half lengths of the register-resident z transforms (kernels_fft.cu: two threads per line)
+template <> struct DFT<18> { DNS_HD static void run(double2 (&x)[18]) { dft_ct<3, 6>(x); } };
+template <> struct DFT<24> { DNS_HD static void run(double2 (&x)[24]) { dft_ct<3, 8>(x); } };
+template <> struct DFT<36> { DNS_HD static void run(double2 (&x)[36]) { dft_ct<6, 6>(x); } };
 
 }  // namespace dnsfft

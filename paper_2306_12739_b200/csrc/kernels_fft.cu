@@ -8,6 +8,8 @@
 //   k_zfwd : mixed -> spectral: forward FFT along z, truncation to the retained modes, 1/(Mx Mz).
 // All FFTs are four-step M = R1*R2 with register codelets (fft_codelets.cuh); the ensemble index is the lane
 // index, so every global access is a contiguous run of members (PAPER.md:167 turned into coalescing).
+#include <cstdlib>
+
 #include "dns_internal.h"
 #include "fft_codelets.cuh"
 
@@ -143,6 +145,117 @@ __global__ void __launch_bounds__(256) k_zfwd(DnsDev d, int etlog, int NB) {
     }
 }
 
+// ------------------------------------------------------------------------------------------------ register versions
+// For Mz = 2H <= 72 a whole z line fits the registers of TWO threads: the pair (lane, lane^1) splits the length-2H
+// transform by one radix-2 step exchanged with warp shuffles, and each thread runs one H-point codelet on its
+// half.  No shared memory, no barrier; every thread has H/1.5 independent 16-byte loads in flight, which is what
+// keeps HBM busy.  Items (kx mode n, member e) of one plane are laid along the lanes, member fastest.
+//   inverse (decimation in time):  thread h transforms the inputs at positions 2i+h;
+//                                  x(k + H h) = E(k) +- w^k O(k), w = exp(-2 pi i / M) on swapped data (swap identity)
+//   forward (decimation in frequency): thread h holds x(i + H h); a_h(i) = (x(i) +- x(i+H)) w^(h i); X(2m + h) = DFT_H(a_h)(m)
+template <int H>
+__global__ void __launch_bounds__(128) k_zinv_r(DnsDev d, const double2* __restrict__ vin) {
+    constexpr int M = 2 * H, LO = H / 3, HI = 2 * H / 3;   // positions 2i+h < M/3 <=> i < LO ; > 2M/3 <=> i > HI (i == HI: h = 1 only)
+    static_assert(H % 3 == 0, "padded length must be 3/2 of an even grid");
+    const int h = threadIdx.x & 1;
+    const int nper = d.nkx * d.E, nblk = (nper + 63) >> 6;
+    const int j = blockIdx.x / nblk + 1;
+    const int q = (blockIdx.x % nblk) * 64 + (threadIdx.x >> 1);
+    const bool ok = q < nper;
+    const int n = ok ? q / d.E : 0, e = ok ? q - n * d.E : 0;
+    const int var = blockIdx.y, f = var < 5 ? var : var - 5;
+    const bool deriv = var >= 5;
+    const double2* src = (f == 0 ? d.uh : f == 1 ? vin : f == 2 ? d.wh : f == 3 ? d.duh : d.dwh) +
+                         ((size_t)j * d.nkx + n) * d.nkz * d.E + e;
+    // all loads first (independent, in flight together), then the i kz factor and the swap of the inverse transform
+    double2 a[H];
+    double kzv[H];
+#pragma unroll
+    for (int i = 0; i < H; ++i) {
+        a[i] = make_double2(0.0, 0.0);
+        kzv[i] = 0.0;
+        if (i < LO || i >= HI) {
+            const int mi = i < LO ? 2 * i + h : 2 * i + h - M / 3 - 1;
+            if (ok && (i != HI || h == 1)) {
+                a[i] = ldg2(src + (size_t)mi * d.E);
+                if (deriv) kzv[i] = __ldg(d.kz + mi);
+            }
+        }
+    }
+    if (deriv) {
+#pragma unroll
+        for (int i = 0; i < H; ++i)
+            if (i < LO || i >= HI) a[i] = make_double2(kzv[i] * a[i].x, -kzv[i] * a[i].y);      // swap(i kz v)
+    } else {
+#pragma unroll
+        for (int i = 0; i < H; ++i)
+            if (i < LO || i >= HI) a[i] = cswap(a[i]);
+    }
+    DFT<H>::run(a);
+    double2* dst = d.I8 + (size_t)var * d.Isz + dns_mix_off(d, j, 0, n, e) + (size_t)(H * h) * ((size_t)(d.ntl * d.nkx) << d.etl);
+    const size_t qs = (size_t)(d.ntl * d.nkx) << d.etl;
+    const double sg = h ? -1.0 : 1.0;
+#pragma unroll
+    for (int k = 0; k < H; ++k) {
+        const double2 o = cmul(a[k], __ldg(d.twz + h * k));
+        double2 r;
+        r.x = __shfl_xor_sync(0xffffffffu, o.x, 1);
+        r.y = __shfl_xor_sync(0xffffffffu, o.y, 1);
+        const double2 x = make_double2(fma(sg, o.x, r.x), fma(sg, o.y, r.y));
+        if (ok) dst[(size_t)k * qs] = cswap(x);
+    }
+}
+
+template <int H>
+__global__ void __launch_bounds__(128) k_zfwd_r(DnsDev d) {
+    constexpr int M = 2 * H, LO = H / 3, HI = 2 * H / 3;
+    const int h = threadIdx.x & 1;
+    const int nper = d.nkx * d.E, nblk = (nper + 63) >> 6;
+    const int j = blockIdx.x / nblk + 1;
+    const int q = (blockIdx.x % nblk) * 64 + (threadIdx.x >> 1);
+    const bool ok = q < nper;
+    const int n = ok ? q / d.E : 0, e = ok ? q - n * d.E : 0;
+    const int f = blockIdx.y;
+    const size_t qs = (size_t)(d.ntl * d.nkx) << d.etl;
+    const double2* src = d.I3 + (size_t)f * d.Isz + dns_mix_off(d, j, 0, n, e) + (size_t)(H * h) * qs;
+    const double sg = h ? -1.0 : 1.0;
+    double2 a[H];
+#pragma unroll
+    for (int i = 0; i < H; ++i) a[i] = ok ? src[(size_t)i * qs] : make_double2(0.0, 0.0);
+#pragma unroll
+    for (int i = 0; i < H; ++i) {
+        double2 r;
+        r.x = __shfl_xor_sync(0xffffffffu, a[i].x, 1);
+        r.y = __shfl_xor_sync(0xffffffffu, a[i].y, 1);
+        const double2 t = make_double2(fma(sg, a[i].x, r.x), fma(sg, a[i].y, r.y));     // x(i) + x(i+H)  |  x(i) - x(i+H)
+        a[i] = cmul(t, __ldg(d.twz + h * i));
+    }
+    DFT<H>::run(a);
+    double2* dst = d.Nh + (size_t)f * d.S + ((size_t)j * d.nkx + n) * d.nkz * d.E + e;
+#pragma unroll
+    for (int m = 0; m < H; ++m) {
+        if (m < LO || m >= HI) {
+            const int mi = m < LO ? 2 * m + h : 2 * m + h - M / 3 - 1;
+            if (ok && (m != HI || h == 1)) dst[(size_t)mi * d.E] = cscale(a[m], d.invMxMz);
+        }
+    }
+}
+
+template <int H> void zinv_r_launch(dns_plan* p, const double2* vin) {
+    const DnsDev& d = p->d;
+    dim3 grid((unsigned)(d.Ni * ((d.nkx * d.E + 63) / 64)), 8);
+    k_zinv_r<H><<<grid, 128, 0, p->stream>>>(d, vin);
+}
+template <int H> void zfwd_r_launch(dns_plan* p) {
+    const DnsDev& d = p->d;
+    dim3 grid((unsigned)(d.Ni * ((d.nkx * d.E + 63) / 64)), 3);
+    k_zfwd_r<H><<<grid, 128, 0, p->stream>>>(d);
+}
+bool use_zreg(int Mz) {
+    static const int off = getenv("DNS_ZREG") ? (atoi(getenv("DNS_ZREG")) == 0) : 0;
+    return !off && (Mz == 24 || Mz == 36 || Mz == 48 || Mz == 72);
+}
+
 template <int R1, int R2> void zinv_launch(dns_plan* p, const double2* vin) {
     const DnsDev& d = p->d;
     const int ET = p->ETf, etlog = __builtin_ctz(ET), M = R1 * R2;
@@ -191,11 +304,27 @@ template <int R1, int R2> void zfwd_launch(dns_plan* p) {
     }
 
 void launch_zinv(dns_plan* p, const double2* vin) {
+    if (use_zreg(p->d.Mz)) {
+        switch (p->d.Mz) {
+            case 24: zinv_r_launch<12>(p, vin); return;
+            case 36: zinv_r_launch<18>(p, vin); return;
+            case 48: zinv_r_launch<24>(p, vin); return;
+            default: zinv_r_launch<36>(p, vin); return;
+        }
+    }
 #define CALL(a, b) zinv_launch<a, b>(p, vin)
     DNS_FFT_DISPATCH(p->d.Mz, CALL)
 #undef CALL
 }
 void launch_zfwd(dns_plan* p) {
+    if (use_zreg(p->d.Mz)) {
+        switch (p->d.Mz) {
+            case 24: zfwd_r_launch<12>(p); return;
+            case 36: zfwd_r_launch<18>(p); return;
+            case 48: zfwd_r_launch<24>(p); return;
+            default: zfwd_r_launch<36>(p); return;
+        }
+    }
 #define CALL(a, b) zfwd_launch<a, b>(p)
     DNS_FFT_DISPATCH(p->d.Mz, CALL)
 #undef CALL
