@@ -82,8 +82,7 @@ __host__ __device__ inline LineSmem line_smem(int R1, int R2, int SL, int TPS, i
     LineSmem s{};
     int off = 0;
     auto take = [&](int bytes) { int o = off; off += (bytes + 127) & ~127; return o; };
-    s.tws_i = take(R2 * SL * 16);
-    s.tws_f = take(R1 * SL * 16);
+    s.tws_i = s.tws_f = 0;
     s.kxs = take(NKX * 8);
     s.group0 = off;
     off = 0;
@@ -108,8 +107,6 @@ __global__ void __launch_bounds__(SL * TPS * NG, MINB) k_line(DnsDev d, int nite
     static_assert(NST == 8 || NST == 4, "ring depth");
     extern __shared__ __align__(128) unsigned char smraw[];
     const LineSmem L = line_smem(R1, R2, SL, TPS, NG, NST);
-    double2* tws_i = reinterpret_cast<double2*>(smraw + L.tws_i);      // [k2][slot] = w_M^(slot k2)
-    double2* tws_f = reinterpret_cast<double2*>(smraw + L.tws_f);      // [k][slot]
     double* kxs = reinterpret_cast<double*>(smraw + L.kxs);
     const int grp = threadIdx.x / GT, t = threadIdx.x % GT;
     unsigned char* gs = smraw + L.group0 + grp * L.group_bytes;
@@ -121,10 +118,9 @@ __global__ void __launch_bounds__(SL * TPS * NG, MINB) k_line(DnsDev d, int nite
     uint64_t* bars = reinterpret_cast<uint64_t*>(gs + L.bars);
 
     const int sl = t / TPS, lis = t % TPS;
+    const double2 om = d.twx[sl % M];                        // w_M^sl
     const int etlog = d.etl, ET = 1 << etlog, el = lis & (ET - 1), lc = lis >> etlog, LC = TPS >> etlog;
     const int ntile = d.ntl, nqg = (d.Mz + LC - 1) / LC;
-    for (int i = threadIdx.x; i < R2 * SL; i += blockDim.x) tws_i[i] = d.twx[((i % SL) * (i / SL)) % M];
-    for (int i = threadIdx.x; i < R1 * SL; i += blockDim.x) tws_f[i] = d.twx[((i % SL) * (i / SL)) % M];
     for (int i = threadIdx.x; i < NKX; i += blockDim.x) kxs[i] = d.kx[i];
     if (t == 0) {
         for (int s = 0; s < NST; ++s) mbar_init(bars + s, 1);
@@ -166,6 +162,12 @@ __global__ void __launch_bounds__(SL * TPS * NG, MINB) k_line(DnsDev d, int nite
         const bool lok = e < E && lc < nl;
         double u[R1], v[R1], w[R1], Nu[R1], Nv[R1], Nw[R1];
         double suv = 0.0, swv = 0.0;
+        // four-step twiddles w_M^(i sl), i < R1: powers of this slot's om = w_M^sl, rebuilt per item from one
+        // register pair instead of R1 + R2 shared-memory reads per transform (the LSU pipe is this kernel's limit)
+        double2 Wp[R1];
+        Wp[0] = make_double2(1.0, 0.0);
+#pragma unroll
+        for (int i = 1; i < R1; ++i) Wp[i] = i == 1 ? om : cmul(Wp[i - 1], om);
 
         // wait for sequence s of this item; refill slot after use with sequence s + NST (this or the next item)
         auto wait_seq = [&](int s) {
@@ -214,7 +216,7 @@ __global__ void __launch_bounds__(SL * TPS * NG, MINB) k_line(DnsDev d, int nite
                 }                                                                                     \
                 DFT<R2>::run(a);                                                                      \
                 _Pragma("unroll")                                                                     \
-                for (int k2 = 0; k2 < R2; ++k2) bufc[sl * PI + k2 * TPS + lis] = cmul(a[k2], tws_i[k2 * SL + sl]); \
+                for (int k2 = 0; k2 < R2; ++k2) bufc[sl * PI + k2 * TPS + lis] = a[k2];               \
             }                                                                                         \
             group_sync<GT>(grp);                                                                      \
             refill(sa);                                                                               \
@@ -222,7 +224,8 @@ __global__ void __launch_bounds__(SL * TPS * NG, MINB) k_line(DnsDev d, int nite
             if (sl < R2) {                                                                            \
                 double2 x[R1];                                                                        \
                 _Pragma("unroll")                                                                     \
-                for (int i1 = 0; i1 < R1; ++i1) x[i1] = bufc[i1 * PI + sl * TPS + lis];               \
+                for (int i1 = 0; i1 < R1; ++i1)                                                       \
+                    x[i1] = i1 ? cmul(bufc[i1 * PI + sl * TPS + lis], Wp[i1]) : bufc[sl * TPS + lis]; \
                 DFT<R1>::run(x);                                                                      \
                 _Pragma("unroll")                                                                     \
                 for (int k = 0; k < R1; ++k) {                                                        \
@@ -253,9 +256,8 @@ __global__ void __launch_bounds__(SL * TPS * NG, MINB) k_line(DnsDev d, int nite
             DFT<R1>::run(a2);
 #pragma unroll
             for (int k = 0; k < R1; ++k) {
-                const double2 tw = tws_f[k * SL + sl];
-                buf0[sl * PF + k * TPS + lis] = cmul(a1[k], tw);
-                buf1[sl * PF + k * TPS + lis] = cmul(a2[k], tw);
+                buf0[sl * PF + k * TPS + lis] = k ? cmul(a1[k], Wp[k]) : a1[k];
+                buf1[sl * PF + k * TPS + lis] = k ? cmul(a2[k], Wp[k]) : a2[k];
             }
             red[sl * TPS + lis] = make_double2(suv, swv);
         }
@@ -341,8 +343,8 @@ template <int R1, int R2, int SL> static void line_launch_tps(dns_plan* p) {
             if constexpr (SL == 8) { line_launch<R1, R2, SL, 4, 4, 8, 3>(p); break; }
         case 8: line_launch<R1, R2, SL, 8, SL == 8 ? 2 : 1, big ? 4 : 8, SL == 8 ? 3 : (big ? 3 : 4)>(p); break;
         default:
-            // small family: ring depth 4 and 128 registers (4 CTAs per SM) measured best on config 2 (155 -> 142 us)
-            if constexpr (SL == 8) line_launch<R1, R2, SL, 16, 1, 4, 4>(p);
+            // small family: ring depth 4 measured best on config 2 (155 -> 141 us); 3 CTAs per SM without spills
+            if constexpr (SL == 8) line_launch<R1, R2, SL, 16, 1, 4, 3>(p);
             else line_launch<R1, R2, SL, 16, 1, big ? 4 : 8, 2>(p);
             break;
     }
