@@ -241,6 +241,108 @@ __global__ void __launch_bounds__(128) k_zfwd_r(DnsDev d) {
     }
 }
 
+// Four threads per line (Mz = 4H = 96): a radix-4 step across the lane quad, done as two radix-2 shuffle stages.
+// Lane (l1, l0) of a quad enters with index 2 l1 + l0 and leaves with index l1 + 2 l0 (the network is its own
+// transpose, so the same code serves the decimation-in-time inverse and the decimation-in-frequency forward).
+__device__ __forceinline__ double2 quad_dft4(double2 z, int l1, int l0) {
+    double2 r;
+    r.x = __shfl_xor_sync(0xffffffffu, z.x, 2);
+    r.y = __shfl_xor_sync(0xffffffffu, z.y, 2);
+    const double s1 = l1 ? -1.0 : 1.0;
+    double2 a = make_double2(fma(s1, z.x, r.x), fma(s1, z.y, r.y));          // l1 = 0: z + partner ; l1 = 1: partner - z
+    if (l0 && l1) a = make_double2(a.y, -a.x);                                 // odd input of the second stage: * (-i)^l1
+    r.x = __shfl_xor_sync(0xffffffffu, a.x, 1);
+    r.y = __shfl_xor_sync(0xffffffffu, a.y, 1);
+    const double s0 = l0 ? -1.0 : 1.0;
+    return make_double2(fma(s0, a.x, r.x), fma(s0, a.y, r.y));
+}
+
+template <int H>
+__global__ void __launch_bounds__(128) k_zinv_r4(DnsDev d, const double2* __restrict__ vin) {
+    constexpr int M = 4 * H, LO = H / 3, HI = 2 * H / 3;   // positions 4i+r < M/3 <=> i < LO ; > 2M/3 <=> i > HI (i == HI: r >= 1)
+    static_assert(H % 3 == 0, "padded length must be 3/2 of an even grid");
+    const int l0 = threadIdx.x & 1, l1 = (threadIdx.x >> 1) & 1, r = 2 * l1 + l0, qo = l1 + 2 * l0;
+    const int nper = d.nkx * d.E, nblk = (nper + 31) >> 5;
+    const int j = blockIdx.x / nblk + 1;
+    const int q = (blockIdx.x % nblk) * 32 + (threadIdx.x >> 2);
+    const bool ok = q < nper;
+    const int n = ok ? q / d.E : 0, e = ok ? q - n * d.E : 0;
+    const int var = blockIdx.y, f = var < 5 ? var : var - 5;
+    const bool deriv = var >= 5;
+    const double2* src = (f == 0 ? d.uh : f == 1 ? vin : f == 2 ? d.wh : f == 3 ? d.duh : d.dwh) +
+                         ((size_t)j * d.nkx + n) * d.nkz * d.E + e;
+    double2 a[H];
+    double kzv[H];
+#pragma unroll
+    for (int i = 0; i < H; ++i) {
+        a[i] = make_double2(0.0, 0.0);
+        kzv[i] = 0.0;
+        if (i < LO || i >= HI) {
+            const int mi = i < LO ? 4 * i + r : 4 * i + r - M / 3 - 1;
+            if (ok && (i != HI || r >= 1)) {
+                a[i] = ldg2(src + (size_t)mi * d.E);
+                if (deriv) kzv[i] = __ldg(d.kz + mi);
+            }
+        }
+    }
+    if (deriv) {
+#pragma unroll
+        for (int i = 0; i < H; ++i)
+            if (i < LO || i >= HI) a[i] = make_double2(kzv[i] * a[i].x, -kzv[i] * a[i].y);      // swap(i kz v)
+    } else {
+#pragma unroll
+        for (int i = 0; i < H; ++i)
+            if (i < LO || i >= HI) a[i] = cswap(a[i]);
+    }
+    DFT<H>::run(a);
+    const size_t qs = (size_t)(d.ntl * d.nkx) << d.etl;
+    double2* dst = d.I8 + (size_t)var * d.Isz + dns_mix_off(d, j, 0, n, e) + (size_t)(H * qo) * qs;
+#pragma unroll
+    for (int k = 0; k < H; ++k) {
+        const double2 x = quad_dft4(cmul(a[k], __ldg(d.twz + r * k)), l1, l0);       // x(k + H qo) on swapped data
+        if (ok) dst[(size_t)k * qs] = cswap(x);
+    }
+}
+
+template <int H>
+__global__ void __launch_bounds__(128) k_zfwd_r4(DnsDev d) {
+    constexpr int M = 4 * H, LO = H / 3, HI = 2 * H / 3;
+    const int l0 = threadIdx.x & 1, l1 = (threadIdx.x >> 1) & 1, qi = 2 * l1 + l0, r = l1 + 2 * l0;
+    const int nper = d.nkx * d.E, nblk = (nper + 31) >> 5;
+    const int j = blockIdx.x / nblk + 1;
+    const int q = (blockIdx.x % nblk) * 32 + (threadIdx.x >> 2);
+    const bool ok = q < nper;
+    const int n = ok ? q / d.E : 0, e = ok ? q - n * d.E : 0;
+    const int f = blockIdx.y;
+    const size_t qs = (size_t)(d.ntl * d.nkx) << d.etl;
+    const double2* src = d.I3 + (size_t)f * d.Isz + dns_mix_off(d, j, 0, n, e) + (size_t)(H * qi) * qs;
+    double2 a[H];
+#pragma unroll
+    for (int i = 0; i < H; ++i) a[i] = ok ? src[(size_t)i * qs] : make_double2(0.0, 0.0);
+#pragma unroll
+    for (int i = 0; i < H; ++i) a[i] = cmul(quad_dft4(a[i], l1, l0), __ldg(d.twz + r * i));
+    DFT<H>::run(a);                                                 // X(4m + r) = a[m]
+    double2* dst = d.Nh + (size_t)f * d.S + ((size_t)j * d.nkx + n) * d.nkz * d.E + e;
+#pragma unroll
+    for (int m = 0; m < H; ++m) {
+        if (m < LO || m >= HI) {
+            const int mi = m < LO ? 4 * m + r : 4 * m + r - M / 3 - 1;
+            if (ok && (m != HI || r >= 1)) dst[(size_t)mi * d.E] = cscale(a[m], d.invMxMz);
+        }
+    }
+}
+
+template <int H> void zinv_r4_launch(dns_plan* p, const double2* vin) {
+    const DnsDev& d = p->d;
+    dim3 grid((unsigned)(d.Ni * ((d.nkx * d.E + 31) / 32)), 8);
+    k_zinv_r4<H><<<grid, 128, 0, p->stream>>>(d, vin);
+}
+template <int H> void zfwd_r4_launch(dns_plan* p) {
+    const DnsDev& d = p->d;
+    dim3 grid((unsigned)(d.Ni * ((d.nkx * d.E + 31) / 32)), 3);
+    k_zfwd_r4<H><<<grid, 128, 0, p->stream>>>(d);
+}
+
 template <int H> void zinv_r_launch(dns_plan* p, const double2* vin) {
     const DnsDev& d = p->d;
     dim3 grid((unsigned)(d.Ni * ((d.nkx * d.E + 63) / 64)), 8);
@@ -253,7 +355,7 @@ template <int H> void zfwd_r_launch(dns_plan* p) {
 }
 bool use_zreg(int Mz) {
     static const int off = getenv("DNS_ZREG") ? (atoi(getenv("DNS_ZREG")) == 0) : 0;
-    return !off && (Mz == 24 || Mz == 36 || Mz == 48 || Mz == 72);
+    return !off && (Mz == 24 || Mz == 36 || Mz == 48 || Mz == 72 || Mz == 96);
 }
 
 template <int R1, int R2> void zinv_launch(dns_plan* p, const double2* vin) {
@@ -309,6 +411,7 @@ void launch_zinv(dns_plan* p, const double2* vin) {
             case 24: zinv_r_launch<12>(p, vin); return;
             case 36: zinv_r_launch<18>(p, vin); return;
             case 48: zinv_r_launch<24>(p, vin); return;
+            case 96: zinv_r4_launch<24>(p, vin); return;
             default: zinv_r_launch<36>(p, vin); return;
         }
     }
@@ -322,6 +425,7 @@ void launch_zfwd(dns_plan* p) {
             case 24: zfwd_r_launch<12>(p); return;
             case 36: zfwd_r_launch<18>(p); return;
             case 48: zfwd_r_launch<24>(p); return;
+            case 96: zfwd_r4_launch<24>(p); return;
             default: zfwd_r_launch<36>(p); return;
         }
     }

@@ -102,7 +102,18 @@ def test_every_transform_length_both_directions(Nx, Nz):
     assert_errs(errs, 2, TOL_1 * 10)
 
 
-@pytest.mark.parametrize("E,Ny,flow", [(1, 17, 0), (5, 20, 1), (33, 12, 0), (7, 5, 1), (2, 66, 1)])
+@pytest.mark.parametrize("Nx,Nz,E", [(48, 32, 17), (32, 48, 9), (32, 32, 21), (64, 16, 19)])
+def test_ragged_member_tiles_of_the_wide_layouts(Nx, Nz, E):
+    """Member tiles of 8 and 16 lanes (line kernel, mixed layout) and the two-thread register z transforms with a
+    ragged last tile / a lane count that is not a multiple of the block; oracle on first, middle and last member."""
+    cfg = inputs.Config(1, inputs.COUETTE, 350.0, 1.9 * PI, 1.1 * PI, Nx, 13, Nz, E, 0.01, 1, 0.1, 0, box=3)
+    members = sorted({0, E // 2, E - 1})
+    errs, _, _ = run_pair(cfg, members, 2, check_at=(1, 2))
+    assert_errs(errs, 1, TOL_1)
+    assert_errs(errs, 2, TOL_1 * 10)
+
+
+@pytest.mark.parametrize("E,Ny,flow", [(1, 17, 0), (5, 20, 1), (33, 12, 0), (7, 5, 1), (2, 66, 1), (6, 75, 0)])
 def test_ragged_members_and_odd_even_ny(E, Ny, flow):
     cfg = inputs.Config(3 if flow else 1, flow, 500.0, 2 * PI, PI, 16, Ny, 12, E, 0.01, 1, 0.1, 0, box=2)
     errs, _, _ = run_pair(cfg, range(E), 3, check_at=(1, 3))
