@@ -4,7 +4,7 @@
   python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--impl reference]
 
 One "step" = one dns_step(1): the whole hot path (3 RK stages x {z-FFT, fused x-line kernel, z-FFT, per-pair DMMA
-kernel, mean flow}) over the whole ensemble of the workload.  At N = 1 the workload is BASELINE.json configs[1]
+kernel with the mean flow in its first CTAs}: 12 launches) over the whole ensemble of the workload.  At N = 1 the workload is BASELINE.json configs[1]
 (plane Couette, Re = 1000, 32 x 49 x 32, E = 64, fp64).  For N > 1 (torchrun, one rank per GPU) every rank advances
 its own 64 members (weak scaling; members are independent, no data-path collective -- SURVEY.md 8(e)).
 Prints ONE JSON line on rank 0 (contract in the task statement): value = whole-job member-steps/s with the state
@@ -180,6 +180,9 @@ def main():
     ap.add_argument("--members", type=int, default=0, help="override E per GPU (config 5 sweep)")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep", action="store_true",
+                    help="BASELINE config 5: one JSON line per ensemble size E in inputs.SWEEP_E (per-kernel times and "
+                         "roofline fractions versus E); not the default bench line")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "b200":
         args.warmup = 3
@@ -198,110 +201,113 @@ def main():
     torch.cuda.set_device(local)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    base = inputs.CONFIGS[args.config]
-    E_gpu = args.members or base.E
-    cfg_all = base.with_E(E_gpu * world)                 # weak scaling: E_gpu members on every rank
-    mine = shard.member_range(cfg_all.E, rank, world)
-    cfg = base.with_E(len(mine))
-    plan = binding.Plan(*inputs.plan_args(cfg), device=f"cuda:{local}")
-    st = inputs.make_state(cfg_all, mine)
-    plan.set_state(st["vhat"], st["etahat"], st["U00"], st["W00"])
-    stream = torch.cuda.current_stream()
+    base = inputs.CONFIGS[5 if args.sweep else args.config]
+    sizes = list(inputs.SWEEP_E) if args.sweep else [args.members or base.E]
+    for E_gpu in sizes:
+        if args.sweep:
+            args.steps, args.warmup = 50, 5                  # BASELINE config 5: 50 steps per ensemble size
+        cfg_all = base.with_E(E_gpu * world)                 # weak scaling: E_gpu members on every rank
+        mine = shard.member_range(cfg_all.E, rank, world)
+        cfg = base.with_E(len(mine))
+        plan = binding.Plan(*inputs.plan_args(cfg), device=f"cuda:{local}")
+        st = inputs.make_state(cfg_all, mine)
+        plan.set_state(st["vhat"], st["etahat"], st["U00"], st["W00"])
+        stream = torch.cuda.current_stream()
 
-    def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
+        def barrier():
+            if world > 1:
+                dist.barrier()
+            torch.cuda.synchronize()
 
-    # ---- device-resident timing: W warm-up steps, then exactly K steps between two events
-    plan.step(args.warmup)
-    barrier()
-    sampler = ClockSampler(local)
-    sampler.start()
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    ev0.record(stream)
-    plan.step(args.steps)
-    ev1.record(stream)
-    barrier()
-    ms = ev0.elapsed_time(ev1)
-    clocks = sampler.stop()
-    ms_max = shard.max_over_ranks(ms) if world > 1 else ms
-    value = cfg_all.E * args.steps / (ms_max * 1e-3)
+        # ---- device-resident timing: W warm-up steps, then exactly K steps between two events
+        plan.step(args.warmup)
+        barrier()
+        sampler = ClockSampler(local)
+        sampler.start()
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev0.record(stream)
+        plan.step(args.steps)
+        ev1.record(stream)
+        barrier()
+        ms = ev0.elapsed_time(ev1)
+        clocks = sampler.stop()
+        ms_max = shard.max_over_ranks(ms) if world > 1 else ms
+        value = cfg_all.E * args.steps / (ms_max * 1e-3)
 
-    # ---- per-kernel-class durations with CUDA events on the same stream (live, same state)
-    nprof = min(max(args.steps // 10, 3), 20)
-    prof = plan.step_profile(nprof)
-    counts = workload_counts(cfg, cfg.E)
-    hbm_peak, peak_src = measured_peaks()
-    kernels = {}
-    for name, msum in prof.items():
-        per_launch_s = msum * 1e-3 / (3 * nprof)
-        c = counts[name]
-        t_hbm, t_alu = c["bytes"] / (hbm_peak * 1e9), c["flops"] / (FP64_PEAK_TFLOPS * 1e12)
-        kernels[name] = {"us_per_launch": per_launch_s * 1e6, "share": msum / max(sum(prof.values()), 1e-30),
-                         "GBps": c["bytes"] / per_launch_s * 1e-9, "TFLOPs": c["flops"] / per_launch_s * 1e-12,
-                         "bound": "hbm" if t_hbm >= t_alu else "fp64",
-                         "frac": max(t_hbm, t_alu) / per_launch_s}
-    dom = max(kernels, key=lambda k: kernels[k]["share"])
-    kd = kernels[dom]
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "dominant_kernel_traffic.json")
-    if os.path.exists(tpath):
-        try:
-            tj = json.load(open(tpath))
-            if tj.get("kernel") == dom and tj.get("workload") == cfg.name:
-                traffic = tj.get("dram_bytes_per_launch")
-        except Exception:
-            traffic = None
-    if kd["bound"] == "hbm":
-        roofline = {"bound": "hbm", "achieved": kd["GBps"], "peak": hbm_peak, "unit": "GB/s",
-                    "frac": kd["GBps"] / hbm_peak, "traffic": traffic}
-    else:
-        roofline = {"bound": "tensor" if dom == "ypair_dmma" else "alu", "achieved": kd["TFLOPs"],
-                    "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": kd["TFLOPs"] / FP64_PEAK_TFLOPS,
-                    "traffic": traffic}
-    roofline.update({"kernel": dom, "peak_source": peak_src + "; fp64 37.0 TFLOP/s measured DMMA/DFMA microbenchmark",
-                     "us_per_launch": kd["us_per_launch"], "share_of_step": kd["share"]})
+        # ---- per-kernel-class durations with CUDA events on the same stream (live, same state)
+        nprof = min(max(args.steps // 10, 3), 20)
+        prof = plan.step_profile(nprof)
+        counts = workload_counts(cfg, cfg.E)
+        hbm_peak, peak_src = measured_peaks()
+        kernels = {}
+        for name, msum in prof.items():
+            per_launch_s = msum * 1e-3 / (3 * nprof)
+            c = counts[name]
+            t_hbm, t_alu = c["bytes"] / (hbm_peak * 1e9), c["flops"] / (FP64_PEAK_TFLOPS * 1e12)
+            kernels[name] = {"us_per_launch": per_launch_s * 1e6, "share": msum / max(sum(prof.values()), 1e-30),
+                             "GBps": c["bytes"] / per_launch_s * 1e-9, "TFLOPs": c["flops"] / per_launch_s * 1e-12,
+                             "bound": "hbm" if t_hbm >= t_alu else "fp64",
+                             "frac": max(t_hbm, t_alu) / per_launch_s}
+        dom = max(kernels, key=lambda k: kernels[k]["share"])
+        kd = kernels[dom]
+        traffic = None
+        tpath = os.path.join(ROOT, "profiles", "dominant_kernel_traffic.json")
+        if os.path.exists(tpath):
+            try:
+                tj = json.load(open(tpath))
+                if tj.get("kernel") == dom and tj.get("workload") == cfg.name:
+                    traffic = tj.get("dram_bytes_per_launch")
+            except Exception:
+                traffic = None
+        if kd["bound"] == "hbm":
+            roofline = {"bound": "hbm", "achieved": kd["GBps"], "peak": hbm_peak, "unit": "GB/s",
+                        "frac": kd["GBps"] / hbm_peak, "traffic": traffic}
+        else:
+            roofline = {"bound": "tensor" if dom == "ypair_dmma" else "alu", "achieved": kd["TFLOPs"],
+                        "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": kd["TFLOPs"] / FP64_PEAK_TFLOPS,
+                        "traffic": traffic}
+        roofline.update({"kernel": dom, "peak_source": peak_src + "; fp64 37.0 TFLOP/s measured DMMA/DFMA microbenchmark",
+                         "us_per_launch": kd["us_per_launch"], "share_of_step": kd["share"]})
 
-    # ---- end to end through the C ABI with HOST (pinned) buffers: H2D + step + D2H every step
-    pin = [torch.from_numpy(np.ascontiguousarray(st[k])).pin_memory() for k in ("vhat", "etahat", "U00", "W00")]
-    outs = [torch.empty_like(t).pin_memory() for t in pin]
-    h2d = sum(t.numel() * t.element_size() for t in pin)
-    d2h = sum(t.numel() * t.element_size() for t in outs)
-    ne2e = min(args.steps, 20)
-    for _ in range(2):
-        plan.set_state(*pin)
-        plan.step(1)
-        plan.get_state(outs)
-    barrier()
-    t0 = time.perf_counter()
-    for _ in range(ne2e):
-        plan.set_state(*pin)
-        plan.step(1)
-        plan.get_state(outs)
-    barrier()
-    e2e_s = time.perf_counter() - t0
-    e2e_s = shard.max_over_ranks(e2e_s) if world > 1 else e2e_s
-    e2e = {"value": cfg_all.E * ne2e / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-           "steps": ne2e, "note": "dns_set_state(host pinned) + dns_step(1) + dns_get_state(host pinned) per step"}
+        # ---- end to end through the C ABI with HOST (pinned) buffers: H2D + step + D2H every step
+        pin = [torch.from_numpy(np.ascontiguousarray(st[k])).pin_memory() for k in ("vhat", "etahat", "U00", "W00")]
+        outs = [torch.empty_like(t).pin_memory() for t in pin]
+        h2d = sum(t.numel() * t.element_size() for t in pin)
+        d2h = sum(t.numel() * t.element_size() for t in outs)
+        ne2e = min(args.steps, 20)
+        for _ in range(2):
+            plan.set_state(*pin)
+            plan.step(1)
+            plan.get_state(outs)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(ne2e):
+            plan.set_state(*pin)
+            plan.step(1)
+            plan.get_state(outs)
+        barrier()
+        e2e_s = time.perf_counter() - t0
+        e2e_s = shard.max_over_ranks(e2e_s) if world > 1 else e2e_s
+        e2e = {"value": cfg_all.E * ne2e / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+               "steps": ne2e, "note": "dns_set_state(host pinned) + dns_step(1) + dns_get_state(host pinned) per step"}
 
-    line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f64", "data": "synthetic",
-        "config": {"workload": cfg.name, "members_per_gpu": cfg.E, "members_total": cfg_all.E,
-                   "parallelism": f"member-shards x{world} (no collective in dns_step)",
-                   "l2_policy": "working set %.0f MB per GPU > 126 MB L2 (no flush needed)" % (plan.workspace_bytes / 1e6)
-                   if plan.workspace_bytes > 2 * 126e6 else "working set fits L2; not flushed between steps (stated)",
-                   "input_sha256": st["sha256"][:16]},
-        "clocks": clocks, "e2e": e2e, "gpu_launches": args.steps * plan.launches_per_step(),
-        "roofline": roofline, "kernels": kernels,
-    }
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        line["cpu_baseline"] = cpu_baseline(base)
-    plan.close()
-    if rank == 0:
-        print(json.dumps(line))
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": cfg.name, "members_per_gpu": cfg.E, "members_total": cfg_all.E,
+                       "parallelism": f"member-shards x{world} (no collective in dns_step)",
+                       "l2_policy": "working set %.0f MB per GPU > 126 MB L2 (no flush needed)" % (plan.workspace_bytes / 1e6)
+                       if plan.workspace_bytes > 2 * 126e6 else "working set fits L2; not flushed between steps (stated)",
+                       "input_sha256": st["sha256"][:16]},
+            "clocks": clocks, "e2e": e2e, "gpu_launches": args.steps * plan.launches_per_step(),
+            "roofline": roofline, "kernels": kernels,
+        }
+        if rank == 0 and world == 1 and not args.no_cpu_baseline and not args.sweep:
+            line["cpu_baseline"] = cpu_baseline(base)
+        plan.close()
+        if rank == 0:
+            print(json.dumps(line))
     if world > 1:
         dist.barrier()
         dist.destroy_process_group()
