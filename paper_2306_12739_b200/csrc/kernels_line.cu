@@ -345,7 +345,7 @@ template <int R1, int R2, int SL> static void line_launch_tps(dns_plan* p) {
         default:
             // small family: ring depth 4 measured best on config 2 (155 -> 141 us); 3 CTAs per SM without spills
             if constexpr (SL == 8) line_launch<R1, R2, SL, 16, 1, 4, 3>(p);
-            else line_launch<R1, R2, SL, 16, 1, big ? 4 : 8, 2>(p);
+            else line_launch<R1, R2, SL, 16, 1, 4, 2>(p);
             break;
     }
 }
