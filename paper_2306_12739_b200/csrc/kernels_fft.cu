@@ -153,7 +153,7 @@ __global__ void __launch_bounds__(256) k_zfwd(DnsDev d, int etlog, int NB) {
 //   inverse (decimation in time):  thread h transforms the inputs at positions 2i+h;
 //                                  x(k + H h) = E(k) +- w^k O(k), w = exp(-2 pi i / M) on swapped data (swap identity)
 //   forward (decimation in frequency): thread h holds x(i + H h); a_h(i) = (x(i) +- x(i+H)) w^(h i); X(2m + h) = DFT_H(a_h)(m)
-template <int H>
+template <int H, bool TP>
 __global__ void __launch_bounds__(128) k_zinv_r(DnsDev d, const double2* __restrict__ vin) {
     constexpr int M = 2 * H, LO = H / 3, HI = 2 * H / 3;   // positions 2i+h < M/3 <=> i < LO ; > 2M/3 <=> i > HI (i == HI: h = 1 only)
     static_assert(H % 3 == 0, "padded length must be 3/2 of an even grid");
@@ -163,10 +163,15 @@ __global__ void __launch_bounds__(128) k_zinv_r(DnsDev d, const double2* __restr
     const int q = (blockIdx.x % nblk) * 64 + (threadIdx.x >> 1);
     const bool ok = q < nper;
     const int n = ok ? q / d.E : 0, e = ok ? q - n * d.E : 0;
-    const int var = blockIdx.y, f = var < 5 ? var : var - 5;
-    const bool deriv = var >= 5;
+    // TP (two passes): blockIdx.y = input field; u, v, w also give their z-derivative in a second pass over the same
+    // inputs (now L1/L2 hits): 3 S less DRAM traffic, more registers.  Otherwise blockIdx.y = one of the 8 outputs.
+    const int f = TP ? blockIdx.y : (blockIdx.y < 5 ? blockIdx.y : blockIdx.y - 5);
     const double2* src = (f == 0 ? d.uh : f == 1 ? vin : f == 2 ? d.wh : f == 3 ? d.duh : d.dwh) +
                          ((size_t)j * d.nkx + n) * d.nkz * d.E + e;
+#pragma unroll 1
+    for (int pass = 0; pass < (TP && f < 3 ? 2 : 1); ++pass) {
+    const bool deriv = TP ? pass == 1 : blockIdx.y >= 5;
+    const int var = TP ? (deriv ? f + 5 : f) : blockIdx.y;
     // all loads first (independent, in flight together), then the i kz factor and the swap of the inverse transform
     double2 a[H];
     double kzv[H];
@@ -203,6 +208,7 @@ __global__ void __launch_bounds__(128) k_zinv_r(DnsDev d, const double2* __restr
         r.y = __shfl_xor_sync(0xffffffffu, o.y, 1);
         const double2 x = make_double2(fma(sg, o.x, r.x), fma(sg, o.y, r.y));
         if (ok) dst[(size_t)k * qs] = cswap(x);
+    }
     }
 }
 
@@ -257,7 +263,7 @@ __device__ __forceinline__ double2 quad_dft4(double2 z, int l1, int l0) {
     return make_double2(fma(s0, a.x, r.x), fma(s0, a.y, r.y));
 }
 
-template <int H>
+template <int H, bool TP>
 __global__ void __launch_bounds__(128) k_zinv_r4(DnsDev d, const double2* __restrict__ vin) {
     constexpr int M = 4 * H, LO = H / 3, HI = 2 * H / 3;   // positions 4i+r < M/3 <=> i < LO ; > 2M/3 <=> i > HI (i == HI: r >= 1)
     static_assert(H % 3 == 0, "padded length must be 3/2 of an even grid");
@@ -267,10 +273,15 @@ __global__ void __launch_bounds__(128) k_zinv_r4(DnsDev d, const double2* __rest
     const int q = (blockIdx.x % nblk) * 32 + (threadIdx.x >> 2);
     const bool ok = q < nper;
     const int n = ok ? q / d.E : 0, e = ok ? q - n * d.E : 0;
-    const int var = blockIdx.y, f = var < 5 ? var : var - 5;
-    const bool deriv = var >= 5;
+    // TP (two passes): blockIdx.y = input field; u, v, w also give their z-derivative in a second pass over the same
+    // inputs (now L1/L2 hits): 3 S less DRAM traffic, more registers.  Otherwise blockIdx.y = one of the 8 outputs.
+    const int f = TP ? blockIdx.y : (blockIdx.y < 5 ? blockIdx.y : blockIdx.y - 5);
     const double2* src = (f == 0 ? d.uh : f == 1 ? vin : f == 2 ? d.wh : f == 3 ? d.duh : d.dwh) +
                          ((size_t)j * d.nkx + n) * d.nkz * d.E + e;
+#pragma unroll 1
+    for (int pass = 0; pass < (TP && f < 3 ? 2 : 1); ++pass) {
+    const bool deriv = TP ? pass == 1 : blockIdx.y >= 5;
+    const int var = TP ? (deriv ? f + 5 : f) : blockIdx.y;
     double2 a[H];
     double kzv[H];
 #pragma unroll
@@ -301,6 +312,7 @@ __global__ void __launch_bounds__(128) k_zinv_r4(DnsDev d, const double2* __rest
     for (int k = 0; k < H; ++k) {
         const double2 x = quad_dft4(cmul(a[k], __ldg(d.twz + r * k)), l1, l0);       // x(k + H qo) on swapped data
         if (ok) dst[(size_t)k * qs] = cswap(x);
+    }
     }
 }
 
@@ -335,7 +347,7 @@ __global__ void __launch_bounds__(128) k_zfwd_r4(DnsDev d) {
 template <int H> void zinv_r4_launch(dns_plan* p, const double2* vin) {
     const DnsDev& d = p->d;
     dim3 grid((unsigned)(d.Ni * ((d.nkx * d.E + 31) / 32)), 8);
-    k_zinv_r4<H><<<grid, 128, 0, p->stream>>>(d, vin);
+    k_zinv_r4<H, false><<<grid, 128, 0, p->stream>>>(d, vin);
 }
 template <int H> void zfwd_r4_launch(dns_plan* p) {
     const DnsDev& d = p->d;
@@ -345,8 +357,9 @@ template <int H> void zfwd_r4_launch(dns_plan* p) {
 
 template <int H> void zinv_r_launch(dns_plan* p, const double2* vin) {
     const DnsDev& d = p->d;
-    dim3 grid((unsigned)(d.Ni * ((d.nkx * d.E + 63) / 64)), 8);
-    k_zinv_r<H><<<grid, 128, 0, p->stream>>>(d, vin);
+    constexpr bool TP = H <= 24;                      // measured: helps Mz <= 48, costs occupancy above
+    dim3 grid((unsigned)(d.Ni * ((d.nkx * d.E + 63) / 64)), TP ? 5 : 8);
+    k_zinv_r<H, TP><<<grid, 128, 0, p->stream>>>(d, vin);
 }
 template <int H> void zfwd_r_launch(dns_plan* p) {
     const DnsDev& d = p->d;
