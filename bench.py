@@ -4,7 +4,7 @@
   python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--impl reference]
 
 One "step" = one dns_step(1): the whole hot path (3 RK stages x {z-FFT, fused x-line kernel, z-FFT, per-pair DMMA
-kernel with the mean flow in its first CTAs}: 12 launches) over the whole ensemble of the workload.  At N = 1 the workload is BASELINE.json configs[1]
+kernel; the mean-flow kernel runs beside the last two on a side stream}: 15 launches) over the whole ensemble.  At N = 1 the workload is BASELINE.json configs[1]
 (plane Couette, Re = 1000, 32 x 49 x 32, E = 64, fp64).  For N > 1 (torchrun, one rank per GPU) every rank advances
 its own 64 members (weak scaling; members are independent, no data-path collective -- SURVEY.md 8(e)).
 Prints ONE JSON line on rank 0 (contract in the task statement): value = whole-job member-steps/s with the state
@@ -109,7 +109,7 @@ def workload_counts(cfg, E):
         "fft_z_fwd": {"bytes": 3 * I + 3 * S, "flops": 3 * Ni * nkx * E * fz},
         # reads Nu,Nv,Nw,v_t,eta_t (+ F,G history), writes v', u, w, du, dw (+ history / eta): ~13 fields, plus the
         # parity-folded matrices (3 per pair, half size); flops of the 7 products in the reflection-parity basis.
-        # The mean flow (row a10) rides in the first CTAs of the same launch: its bytes are added here.
+        # The mean flow (row a10) runs on a side stream under this class's events: its bytes are added here.
         "ypair_dmma": {"bytes": 13 * S + 3 * (Kh * Kh + Kho * Kho) * 8.0 * nmat + Ni * Mz * E * 16.0 + 12 * cfg.Ny * E * 8.0,
                        "flops": 7 * 2.0 * (Kh * Kh + Kho * Kho) * 2 * E * (P - 1)},
     }

@@ -53,7 +53,8 @@ enum {
     DNS_CLASS_LINE = 1,      /* a4 x direction + a5 products + a6 x direction, fused per (y,z) line */
     DNS_CLASS_FFT_Z_FWD = 2, /* a6, z direction: forward FFT + truncation + 1/(Mx Mz)              */
     DNS_CLASS_YPAIR = 3,     /* a7,a8,a9,a1,a2,a3: per-(kx,kz) DMMA contractions + stage algebra;
-                                a10 (mean flow, wall lift, mass-flux gamma) runs in the first CTAs of the same launch */
+                                a10 (mean flow, wall lift, mass-flux gamma) is a small kernel on an internal side stream
+                                that runs under classes 2 and 3 and is joined before this class's closing event */
     DNS_NCLASS = 4
 };
 

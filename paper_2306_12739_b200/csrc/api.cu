@@ -70,10 +70,16 @@ void run_stage(dns_plan* p, int s, cudaEvent_t* ev) {
     launch_zinv(p, vin);
     if (ev) cudaEventRecord(ev[1], p->stream);
     launch_line(p);
+    // the mean flow (row a10) needs only the plane sums of the line kernel: fork it onto the side stream, join at the end
+    cudaEventRecord(p->ev_fork, p->stream);
+    cudaStreamWaitEvent(p->side, p->ev_fork, 0);
+    launch_mean(p, s, 0, p->side);
+    cudaEventRecord(p->ev_join, p->side);
     if (ev) cudaEventRecord(ev[2], p->stream);
     launch_zfwd(p);
     if (ev) cudaEventRecord(ev[3], p->stream);
     launch_ypair(p, s, 0);
+    cudaStreamWaitEvent(p->stream, p->ev_join, 0);
     if (ev) cudaEventRecord(ev[4], p->stream);
 }
 
@@ -138,6 +144,13 @@ int dns_plan_create(dns_plan** out, int Nx, int Ny, int Nz, int E, double Re, do
     p->NTy = ETy >= 8 ? 2 : 1;
     if (const char* s = getenv("DNS_NTY")) { int v = atoi(s); if ((v == 1 || v == 2 || v == 4) && 4 * v <= ETy) p->NTy = v; }
     while (32 * (d.Kp / 8) * (ETy / (4 * p->NTy)) > 1024) p->NTy *= 2;
+    if (cudaStreamCreateWithFlags(&p->side, cudaStreamNonBlocking) != cudaSuccess ||
+        cudaEventCreateWithFlags(&p->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&p->ev_join, cudaEventDisableTiming) != cudaSuccess) {
+        cudaGetLastError();
+        dns_plan_destroy(p);
+        return DNS_ECUDA;
+    }
     int st = DNS_OK;
     try {
         st = dns_host_precompute(p);
@@ -188,7 +201,8 @@ int dns_set_state(dns_plan* p, const double* vhat, const double* etahat, const d
     launch_abi_to_internal(p, se, d.et);
     launch_normalise_state(p);
     launch_mean_in(p, sU, sW);
-    launch_ypair(p, 0, 1);          // derive u, w, du/dy, dw/dy of the initial state (Eq. 17-18), incl. the (0,0) column
+    launch_ypair(p, 0, 1);          // derive u, w, du/dy, dw/dy of the initial state (Eq. 17-18)
+    launch_mean(p, 0, 1, p->stream);   // and their (0,0) column
     p->has_state = true;
     p->nsteps_done = 0;
     e = cudaGetLastError();
@@ -310,11 +324,14 @@ int dns_debug_stage(dns_plan* p, int stage) {
     return cuda_status(p, cudaGetLastError());
 }
 
-int dns_launches_per_step(const dns_plan* p) { return p ? 3 * 4 : 0; }
+int dns_launches_per_step(const dns_plan* p) { return p ? 3 * 5 : 0; }
 
 int dns_plan_destroy(dns_plan* p) {
     if (!p) return DNS_OK;
     for (void* q : p->owned) cudaFree(q);
+    if (p->side) cudaStreamDestroy(p->side);
+    if (p->ev_fork) cudaEventDestroy(p->ev_fork);
+    if (p->ev_join) cudaEventDestroy(p->ev_join);
     if (p->ev_init)
         for (auto& e : p->ev) cudaEventDestroy(e);
     delete p;

@@ -61,6 +61,8 @@ struct dns_plan {
     int line_grid = 0;                         // persistent grid of the line kernel (set at first launch)
     int line_tps = 0;                          // lanes per slot of the line kernel (4, 8 or 16)
     alignas(64) unsigned char tmaps[3][128];   // CUtensorMap of Nh, vt, et (encoded at dns_plan_bind)
+    cudaStream_t side = nullptr;               // the mean-flow kernel runs here, under the z-forward and per-pair kernels
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
     std::vector<void*> owned;                  // plan-owned device allocations
     void* workspace = nullptr;
     size_t workspace_bytes = 0;
@@ -84,6 +86,7 @@ void launch_zfwd(dns_plan* p);
 void launch_ypair(dns_plan* p, int stage, int derive_only);
 size_t dns_ypair_smem(int Ni, int Ny, int ET);
 int dns_ypair_encode_maps(dns_plan* p);
+void launch_mean(dns_plan* p, int stage, int derive_only, cudaStream_t stream);
 void launch_abi_to_internal(dns_plan* p, const double2* src_abi, double2* dst);
 void launch_internal_to_abi(dns_plan* p, const double2* src, double2* dst_abi);
 void launch_mean_in(dns_plan* p, const double* U_abi, const double* W_abi);

@@ -93,9 +93,35 @@ __device__ __forceinline__ void st2(double* p, double2 v) { *reinterpret_cast<do
 
 // ------------------------------------------------------------------------------------------------ mean flow
 // CTA-wide: tiles of 8 members x (blockDim/8) row slots; dynamic smem = 6 vectors [Ny][8]
+// sa += sum_k M[k] xa[8 k + el], sb likewise with xb, k in [k0, k1) in ascending order.  The 8 member lanes of a row slot
+// need the same matrix row: each loads one eighth of it (all loads of a 64-column chunk in flight at once) and the
+// values are handed round with shuffles, so a row costs one memory round trip instead of one per four columns.
+// Must be called by all 32 lanes with the same k0, k1 (Mrow may differ per row slot).
+__device__ __forceinline__ void rowdot2(const double* __restrict__ Mrow, int k0, int k1, const double* xa, const double* xb,
+                                        int el, int lane, double& sa, double& sb) {
+    for (int base = k0; base < k1; base += 64) {
+        double c[8];
+#pragma unroll
+        for (int m = 0; m < 8; ++m) {
+            const int kk = base + 8 * m + el;
+            c[m] = kk < k1 ? __ldg(Mrow + kk) : 0.0;
+        }
+#pragma unroll
+        for (int m = 0; m < 8; ++m) {
+            if (base + 8 * m >= k1) break;
+#pragma unroll
+            for (int s8 = 0; s8 < 8; ++s8) {
+                const double v = __shfl_sync(0xffffffffu, c[m], (lane & 24) + s8);
+                const int k = base + 8 * m + s8;
+                if (k < k1) { sa += v * xa[k * 8 + el]; sb += v * xb[k * 8 + el]; }
+            }
+        }
+    }
+}
+
 __device__ void mean_body(const DnsDev& d, int stage, int derive_only, int tile, double* smm) {
     const int Ny = d.Ny, Ni = d.Ni, nrs = blockDim.x >> 3;
-    const int el = threadIdx.x & 7, rs = threadIdx.x >> 3, e = tile * 8 + el;
+    const int el = threadIdx.x & 7, rs = threadIdx.x >> 3, e = tile * 8 + el, lane = threadIdx.x & 31;
     const bool eok = e < d.E;
     const int hi = stage == 0 ? 0 : 1;
     const double hdt = (stage == 0 ? 0.5 : 1.0) * d.dt;
@@ -110,12 +136,17 @@ __device__ void mean_body(const DnsDev& d, int stage, int derive_only, int tile,
     double* Wout = stage == 2 ? d.Wt : d.Ws;
     if (!derive_only) {
         // plane means [uv]00, [wv]00 (Eq. 6-7): fixed-order sum of the per-line partial sums
-        for (int j = rs; j < Ny; j += nrs) {
+        if (threadIdx.x < 16) { const int w = threadIdx.x >> 3; uvc[w * (Ny - 1) * 8 + el] = 0.0; wvc[w * (Ny - 1) * 8 + el] = 0.0; }   // wall rows
+        for (int j = 1 + rs; j < Ny - 1; j += nrs) {
             double a = 0.0, b = 0.0;
-            if (eok && j > 0 && j < Ny - 1) {
-                for (int q = 0; q < d.Mz; ++q) {
-                    const double2 v = d.uvpart[((size_t)j * d.Mz + q) * d.E + e];
-                    a += v.x; b += v.y;
+            if (eok) {
+                const double2* src = d.uvpart + (size_t)j * d.Mz * d.E + e;
+                for (int q0 = 0; q0 < d.Mz; q0 += 16) {          // 16 loads in flight, summed in ascending q
+                    double2 v[16];
+#pragma unroll
+                    for (int u = 0; u < 16; ++u) v[u] = q0 + u < d.Mz ? src[(size_t)(q0 + u) * d.E] : make_double2(0.0, 0.0);
+#pragma unroll
+                    for (int u = 0; u < 16; ++u) { a += v[u].x; b += v[u].y; }
                 }
                 a *= d.invMxMz; b *= d.invMxMz;
                 // history: stage 0 stores S0, stage 1 replaces it by S0 + 4 S1
@@ -128,22 +159,26 @@ __device__ void mean_body(const DnsDev& d, int stage, int derive_only, int tile,
         }
         __syncthreads();
         // rhs = 2 U_t - h dt D [uv] - 2 bc  (Eq. 14 with S0p = 2I - S0m and the wall columns on the rhs)
-        for (int i = rs; i < Ni; i += nrs) {
+        for (int i0 = 0; i0 < Ni; i0 += nrs) {                    // all lanes run every round (shuffles inside rowdot2)
+            const int i = i0 + rs < Ni ? i0 + rs : Ni - 1;
             double su = 0.0, sw = 0.0;
-            const double* Dr = d.Dfull + (size_t)(i + 1) * Ny;
-            for (int j = 1; j < Ny - 1; ++j) { su += Dr[j] * uvc[j * 8 + el]; sw += Dr[j] * wvc[j * 8 + el]; }
+            rowdot2(d.Dfull + (size_t)(i + 1) * Ny, 1, Ny - 1, uvc, wvc, el, lane, su, sw);
             const double ut = eok ? d.Ut[(size_t)(i + 1) * d.E + e] : 0.0, wt = eok ? d.Wt[(size_t)(i + 1) * d.E + e] : 0.0;
-            ru[i * 8 + el] = 2.0 * ut - hdt * su - 2.0 * d.bc[hi * Ni + i];
-            rw[i * 8 + el] = 2.0 * wt - hdt * sw;
+            if (i0 + rs < Ni) {
+                ru[i * 8 + el] = 2.0 * ut - hdt * su - 2.0 * d.bc[hi * Ni + i];
+                rw[i * 8 + el] = 2.0 * wt - hdt * sw;
+            }
         }
         __syncthreads();
-        for (int i = rs; i < Ni; i += nrs) {
+        for (int i0 = 0; i0 < Ni; i0 += nrs) {
+            const int i = i0 + rs < Ni ? i0 + rs : Ni - 1;
             double su = 0.0, sw = 0.0;
-            const double* Sr = d.S0inv + (size_t)hi * Ni * Ni + (size_t)i * Ni;
-            for (int k = 0; k < Ni; ++k) { su += Sr[k] * ru[k * 8 + el]; sw += Sr[k] * rw[k * 8 + el]; }
+            rowdot2(d.S0inv + (size_t)hi * Ni * Ni + (size_t)i * Ni, 0, Ni, ru, rw, el, lane, su, sw);
             const double ut = eok ? d.Ut[(size_t)(i + 1) * d.E + e] : 0.0, wt = eok ? d.Wt[(size_t)(i + 1) * d.E + e] : 0.0;
-            Un[(i + 1) * 8 + el] = su - ut;
-            Wn[(i + 1) * 8 + el] = sw - wt;
+            if (i0 + rs < Ni) {
+                Un[(i + 1) * 8 + el] = su - ut;
+                Wn[(i + 1) * 8 + el] = sw - wt;
+            }
         }
         if (rs == 0) { Un[el] = -d.Uw; Un[(Ny - 1) * 8 + el] = d.Uw; Wn[el] = 0.0; Wn[(Ny - 1) * 8 + el] = 0.0; }
         __syncthreads();
@@ -173,11 +208,11 @@ __device__ void mean_body(const DnsDev& d, int stage, int derive_only, int tile,
         __syncthreads();
     }
     // (0,0) column of the transform inputs: u = U00, w = W00, du/dy = D U00, dw/dy = D W00
-    for (int j = rs; j < Ny; j += nrs) {
+    for (int j0 = 0; j0 < Ny; j0 += nrs) {
+        const int j = j0 + rs < Ny ? j0 + rs : Ny - 1;
         double du = 0.0, dw = 0.0;
-        const double* Dr = d.Dfull + (size_t)j * Ny;
-        for (int k = 0; k < Ny; ++k) { du += Dr[k] * Un[k * 8 + el]; dw += Dr[k] * Wn[k * 8 + el]; }
-        if (eok) {
+        rowdot2(d.Dfull + (size_t)j * Ny, 0, Ny, Un, Wn, el, lane, du, dw);
+        if (eok && j0 + rs < Ny) {
             const size_t gi = ((size_t)j * d.P) * d.E + e;
             d.uh[gi] = make_double2(Un[j * 8 + el], 0.0);
             d.wh[gi] = make_double2(Wn[j * 8 + el], 0.0);
@@ -201,11 +236,10 @@ constexpr int ypair_minb(int threads) {
 template <int NT, int NWNT, int KS2T>
 __global__ void __launch_bounds__(KS2T ? 32 * KS2T * NWNT : 1024, ypair_minb(32 * KS2T * NWNT))
 k_ypair(DnsDev d, const __grid_constant__ CUtensorMap tmN, const __grid_constant__ CUtensorMap tmV,
-        const __grid_constant__ CUtensorMap tmE, int stage, int derive_only, int nmean) {
+        const __grid_constant__ CUtensorMap tmE, int stage, int derive_only) {
     extern __shared__ __align__(128) double smy[];
     __shared__ uint64_t bar;
-    if ((int)blockIdx.x < nmean) { mean_body(d, stage, derive_only, blockIdx.x, smy); return; }
-    const int bid = blockIdx.x - nmean;
+    const int bid = blockIdx.x;
     const int Ni = d.Ni, KS2 = KS2T ? KS2T : (d.Kp >> 3), Kp = 8 * KS2, Kh = (Ni + 1) >> 1, Kho = Ni >> 1;
     constexpr int NWN = NWNT, NC = 8 * NT * NWN, ET = NC >> 1, ld = NC + 4;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
@@ -474,6 +508,13 @@ k_ypair(DnsDev d, const __grid_constant__ CUtensorMap tmN, const __grid_constant
     }
 }
 
+// mean flow as its own small launch (8 members per CTA); api.cu runs it on a side stream under the z-forward and
+// per-pair kernels: it needs only the plane sums written by the line kernel
+__global__ void __launch_bounds__(256) k_mean(DnsDev d, int stage, int derive_only) {
+    extern __shared__ __align__(128) double smm[];
+    mean_body(d, stage, derive_only, blockIdx.x, smm);
+}
+
 // ------------------------------------------------------------------------------------------------ layout / IO
 // ABI [E][P][Ny] <-> internal [Ny][P][E]; grid = (P, ceil(E/32), ceil(Ny/32)), block = (32, 8)
 __global__ void k_abi_to_internal(const double2* __restrict__ src, double2* __restrict__ dst, int Ny, int P, int E) {
@@ -579,8 +620,8 @@ __global__ void k_diag_rows(DnsDev d, const double* __restrict__ part, double t)
 }  // namespace
 
 size_t dns_ypair_smem(int Ni, int Ny, int ET) {
-    const size_t panels = 5 * ((((size_t)Ni * (2 * ET + 4) + 15) & ~(size_t)15) * sizeof(double)), mean = (size_t)6 * Ny * 8 * sizeof(double);
-    return panels > mean ? panels : mean;
+    (void)Ny;
+    return 5 * ((((size_t)Ni * (2 * ET + 4) + 15) & ~(size_t)15) * sizeof(double));
 }
 
 // TMA descriptors of the per-pair kernel's inputs: 2-D views [rows][2 P E doubles] of the spectral arrays with a
@@ -615,8 +656,7 @@ int dns_ypair_encode_maps(dns_plan* p) {
 template <int NT, int NWN> static void ypair_launch(dns_plan* p, int stage, int derive_only) {
     const DnsDev& d = p->d;
     const int KS2 = d.Kp >> 3, ET = 4 * NT * NWN;
-    const int nmean = (d.E + 7) / 8;
-    const unsigned grid = (unsigned)(nmean + (d.P - 1) * ((d.E + ET - 1) / ET));
+    const unsigned grid = (unsigned)((d.P - 1) * ((d.E + ET - 1) / ET));
     const size_t smem = dns_ypair_smem(d.Ni, d.Ny, ET);
 #define LAUNCH(K)                                                                                     \
     {                                                                                                 \
@@ -624,7 +664,7 @@ template <int NT, int NWN> static void ypair_launch(dns_plan* p, int stage, int 
         cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);           \
         cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared); \
         const CUtensorMap* tm = reinterpret_cast<const CUtensorMap*>(p->tmaps);                       \
-        kern<<<grid, 32 * KS2 * NWN, smem, p->stream>>>(d, tm[0], tm[1], tm[2], stage, derive_only, nmean); \
+        kern<<<grid, 32 * KS2 * NWN, smem, p->stream>>>(d, tm[0], tm[1], tm[2], stage, derive_only); \
     }
     switch (KS2) {
         case 2: LAUNCH(2) break;
@@ -644,6 +684,12 @@ void launch_ypair(dns_plan* p, int stage, int derive_only) {
     else if (NT == 2 && NWN == 2) ypair_launch<2, 2>(p, stage, derive_only);
     else if (NT == 4 && NWN == 1) ypair_launch<4, 1>(p, stage, derive_only);
     else ypair_launch<1, 4>(p, stage, derive_only);
+}
+
+void launch_mean(dns_plan* p, int stage, int derive_only, cudaStream_t stream) {
+    const DnsDev& d = p->d;
+    const size_t smem = (size_t)6 * d.Ny * 8 * sizeof(double);
+    k_mean<<<(d.E + 7) / 8, 256, smem, stream>>>(d, stage, derive_only);
 }
 
 void launch_abi_to_internal(dns_plan* p, const double2* src, double2* dst) {
