@@ -95,7 +95,9 @@ int dns_set_state(dns_plan* plan, const double* vhat, const double* etahat, cons
                   const double* W00);
 
 /* dns_step -- enqueue nsteps full CN/RK3 time steps (3 stages each) on the plan's stream
- * and return without synchronising.  Errors: DNS_EINVAL (nsteps < 0), DNS_ESTATE (no state), DNS_ECUDA. */
+ * and return without synchronising.  The 15 launches of a step are captured once into a CUDA graph (on an internal
+ * stream, at the first call after dns_plan_bind) and replayed per step; DNS_GRAPH=0 in the environment, or a failed
+ * capture, falls back to direct launches with identical results.  Errors: DNS_EINVAL (nsteps < 0), DNS_ESTATE (no state), DNS_ECUDA. */
 int dns_step(dns_plan* plan, int nsteps);
 
 /* dns_step_profile -- as dns_step, but brackets every kernel class with CUDA events on the plan's stream,

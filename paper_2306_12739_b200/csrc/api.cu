@@ -83,6 +83,36 @@ void run_stage(dns_plan* p, int s, cudaEvent_t* ev) {
     if (ev) cudaEventRecord(ev[4], p->stream);
 }
 
+// Captures one time step into a CUDA graph (on an internal stream: the plan's stream may be the legacy default stream,
+// which cannot be captured).  On any failure the plan falls back to direct launches for good.
+void build_step_graph(dns_plan* p) {
+    p->graph_state = -1;
+    if (getenv("DNS_GRAPH") && atoi(getenv("DNS_GRAPH")) == 0) return;
+    if (cudaGetLastError() != cudaSuccess) return;
+    if (!p->capture_stream && cudaStreamCreateWithFlags(&p->capture_stream, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); return; }
+    cudaStream_t user = p->stream;
+    if (cudaStreamBeginCapture(p->capture_stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { cudaGetLastError(); return; }
+    p->stream = p->capture_stream;
+    for (int s = 0; s < 3; ++s) run_stage(p, s, nullptr);
+    p->stream = user;
+    cudaGraph_t g = nullptr;
+    const cudaError_t e1 = cudaStreamEndCapture(p->capture_stream, &g);
+    if (e1 != cudaSuccess || !g) { cudaGetLastError(); return; }
+    cudaGraphExec_t ge = nullptr;
+    if (cudaGraphInstantiate(&ge, g, 0) != cudaSuccess || !ge) { cudaGetLastError(); cudaGraphDestroy(g); return; }
+    p->graph = g;
+    p->graph_exec = ge;
+    p->graph_state = 1;
+}
+
+void drop_step_graph(dns_plan* p) {
+    if (p->graph_exec) cudaGraphExecDestroy(p->graph_exec);
+    if (p->graph) cudaGraphDestroy(p->graph);
+    p->graph_exec = nullptr;
+    p->graph = nullptr;
+    p->graph_state = 0;
+}
+
 }  // namespace
 
 extern "C" {
@@ -173,6 +203,7 @@ int dns_plan_bind(dns_plan* p, void* ws, size_t bytes, void* stream) {
     p->workspace = ws;
     p->stream = static_cast<cudaStream_t>(stream);
     carve_workspace(p, ws);
+    drop_step_graph(p);                                  // the graph holds the old workspace pointers and tensor maps
     const int st = dns_ypair_encode_maps(p);
     if (st != DNS_OK) { p->sticky = st; return st; }
     p->bound = true;
@@ -214,8 +245,13 @@ int dns_step(dns_plan* p, int nsteps) {
     if (!p || nsteps < 0) return DNS_EINVAL;
     if (p->sticky != DNS_OK) return p->sticky;
     if (!p->bound || !p->has_state) return DNS_ESTATE;
+    if (p->graph_state == 0 && nsteps > 0) build_step_graph(p);
     for (int it = 0; it < nsteps; ++it) {
-        for (int s = 0; s < 3; ++s) run_stage(p, s, nullptr);
+        if (p->graph_state == 1) {
+            if (cudaGraphLaunch(p->graph_exec, p->stream) != cudaSuccess) return cuda_status(p, cudaGetLastError());
+        } else {
+            for (int s = 0; s < 3; ++s) run_stage(p, s, nullptr);
+        }
         ++p->nsteps_done;
     }
     return cuda_status(p, cudaGetLastError());
@@ -329,6 +365,8 @@ int dns_launches_per_step(const dns_plan* p) { return p ? 3 * 5 : 0; }
 int dns_plan_destroy(dns_plan* p) {
     if (!p) return DNS_OK;
     for (void* q : p->owned) cudaFree(q);
+    drop_step_graph(p);
+    if (p->capture_stream) cudaStreamDestroy(p->capture_stream);
     if (p->side) cudaStreamDestroy(p->side);
     if (p->ev_fork) cudaEventDestroy(p->ev_fork);
     if (p->ev_join) cudaEventDestroy(p->ev_join);

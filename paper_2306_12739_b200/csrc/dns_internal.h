@@ -68,6 +68,12 @@ struct dns_plan {
     size_t workspace_bytes = 0;
     cudaStream_t stream = nullptr;
     bool bound = false, has_state = false;
+    // one time step (15 launches, fork/join with the side stream) captured once into a CUDA graph and replayed:
+    // small ensembles are launch-bound.  graph_state: 0 not tried, 1 ready, -1 unavailable (direct launches)
+    cudaStream_t capture_stream = nullptr;
+    cudaGraph_t graph = nullptr;
+    cudaGraphExec_t graph_exec = nullptr;
+    int graph_state = 0;
     int sticky = DNS_OK;
     long long nsteps_done = 0;
     cudaEvent_t ev[2 * 16] = {};
