@@ -190,6 +190,31 @@ def test_step_n_equals_n_steps_and_is_deterministic():
             assert np.array_equal(a, b)
 
 
+def test_graph_replay_equals_direct_launches_bitwise(monkeypatch):
+    """dns_step replays a CUDA graph of one time step; DNS_GRAPH=0 and dns_step_profile launch the same kernels directly.
+    All three must give bit-identical states (same kernels, same order, the mean-flow kernel joined before its readers)."""
+    cfg = inputs.CONFIGS[2].with_E(9)
+    st = inputs.make_state(cfg)
+    outs = []
+    for mode in ("graph", "direct", "profile"):
+        if mode == "direct":
+            monkeypatch.setenv("DNS_GRAPH", "0")
+        else:
+            monkeypatch.delenv("DNS_GRAPH", raising=False)
+        plan = binding.Plan(*inputs.plan_args(cfg))
+        plan.set_state(st["vhat"], st["etahat"], st["U00"], st["W00"])
+        if mode == "profile":
+            plan.step_profile(4)
+        else:
+            plan.step(3)
+            plan.step(1)
+        outs.append(plan.get_state())
+        plan.close()
+    for o in outs[1:]:
+        for a, b in zip(outs[0], o):
+            assert np.array_equal(a, b)
+
+
 def test_set_state_normalisation_matches_oracle():
     cfg = inputs.CONFIGS[1]
     st = inputs.make_state(cfg)
