@@ -149,7 +149,10 @@ __global__ void __launch_bounds__(SL * TPS * NG, MINB) k_line(DnsDev d, int nite
     };
 
     int it = blockIdx.x * NG + grp;
-    if (t == 0 && it < nitems)
+    // the thread that issues the bulk copies sits in a warp whose slots are idle in the first pass of the inverse
+    // transforms (slots >= R1), when there is one: the refills then delay nobody on the way to the next group barrier
+    constexpr int LEADER = (TPS * (SL - R1) >= 32 && GT > 32) ? GT - 32 : 0;
+    if (t == LEADER && it < nitems)
         for (int s = 0; s < NST; ++s) issue(it, s);
     uint32_t itc = 0;                                        // items done by this group
 
@@ -175,7 +178,7 @@ __global__ void __launch_bounds__(SL * TPS * NG, MINB) k_line(DnsDev d, int nite
             mbar_wait(bars + (s % NST), use & 1);
         };
         auto refill = [&](int s) {
-            if (t != 0) return;
+            if (t != LEADER) return;
             if (NST == 4 && s < 4) issue(it, s + 4);
             else if (nxt < nitems) issue(nxt, NST == 8 ? s : s - 4);
         };
