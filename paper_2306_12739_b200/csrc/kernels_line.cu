@@ -295,12 +295,12 @@ __global__ void __launch_bounds__(SL * TPS * NG, MINB) k_line(DnsDev d, int nite
                     dst[2 * fstride + (n << etlog)] = n == 0 ? make_double2(x2[k].x, 0.0) : x2[k];
                 }
             }
-            if (sl == 0) {
-                double sa = 0.0, sb = 0.0;
+        }
+        if (sl == SL - 1 && lok) {                           // plane sums: by the last slot, idle in this pass when SL > R1
+            double sa = 0.0, sb = 0.0;
 #pragma unroll
-                for (int s = 0; s < R2; ++s) { sa += red[s * TPS + lis].x; sb += red[s * TPS + lis].y; }
-                d.uvpart[((size_t)j * d.Mz + q) * E + e] = make_double2(sa, sb);
-            }
+            for (int s = 0; s < R2; ++s) { sa += red[s * TPS + lis].x; sb += red[s * TPS + lis].y; }
+            d.uvpart[((size_t)j * d.Mz + q) * E + e] = make_double2(sa, sb);
         }
     }
 }
