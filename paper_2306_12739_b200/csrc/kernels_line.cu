@@ -9,8 +9,9 @@
 // Nothing in physical space ever reaches HBM.
 //
 // Thread mapping: a line is shared by SL "slots"; every slot owns R1 x-points of each physical field in registers.
-// A "group" = SL slots x TPS lanes (lanes = members, or members x lines when E < TPS) = 1..3 warps; the four-step
-// exchanges need only a group-local barrier.  Groups are persistent: each walks over work items (j, q-group, member
+// A "group" = SL slots x TPS lanes (lanes = members, or members x lines when E < TPS; TPS = 4, 8 or 16 by ensemble
+// size) = 1..6 warps; the four-step exchanges need only a group-local barrier.  The four-step twiddles are powers of
+// one per-slot register value, and the thread that issues the bulk copies sits in a warp that idles in the first pass.  Groups are persistent: each walks over work items (j, q-group, member
 // tile).  The mixed arrays are stored tile-major ([j][q][tile][kx][ET]) so that the input of one item and one field
 // is ONE contiguous block, fetched by a single TMA bulk copy (cp.async.bulk + mbarrier) into a ring of field slots
 // one item ahead of the arithmetic: global latency never touches the register file or the LSU pipe.
@@ -73,7 +74,7 @@ __device__ __forceinline__ constexpr int seq_field(int s) {
 template <int C> struct LineSeq { static constexpr int sa = C < 3 ? C : (C == 3 ? 3 : (C == 4 ? 5 : 7)), two = (C == 3 || C == 4); };
 
 struct LineSmem {                     // byte offsets inside the dynamic shared memory of a CTA
-    int tws_i, tws_f, kxs, group0, group_bytes, ring, buf, exch, red, bars, total;
+    int kxs, group0, group_bytes, ring, buf, exch, red, bars, total;
 };
 __host__ __device__ inline LineSmem line_smem(int R1, int R2, int SL, int TPS, int NG, int NST) {
     const int M = R1 * R2, NKX = M / 3;
@@ -82,7 +83,6 @@ __host__ __device__ inline LineSmem line_smem(int R1, int R2, int SL, int TPS, i
     LineSmem s{};
     int off = 0;
     auto take = [&](int bytes) { int o = off; off += (bytes + 127) & ~127; return o; };
-    s.tws_i = s.tws_f = 0;
     s.kxs = take(NKX * 8);
     s.group0 = off;
     off = 0;

@@ -7,9 +7,11 @@
 //             with J the reversal y -> -y of the interior Gauss-Lobatto points, the Chebyshev matrix obeys
 //             J D J = -D and every solve matrix J M J = M, so in the variables s = x + Jx, dd = x - Jx each
 //             [Ni x Ni] product splits into two [Ni/2 x Ni/2] ones: half the flops and half the matrix bytes.
-//             The first CTAs of the grid do the mean flow instead (row a10): U00, W00 of Eq. 14-15 with the wall
-//             lift f+-  and the mass-flux pressure gamma solved so that the discrete bulk flux is
-//             held; they run in the shadow of the pair CTAs.
+//             Inputs arrive as TMA tensor-map tiles (one per field: Ni rows x one member tile, landing in the padded
+//             panel layout).
+//   k_mean  : mean flow (row a10): U00, W00 of Eq. 14-15 with the wall lift f+-  and the mass-flux
+//             pressure gamma solved so that the discrete bulk flux is held; api.cu runs it on a
+//             side stream under the z-forward and per-pair kernels.
 // plus layout conversion, input normalisation and diagnostics.
 #include <cuda.h>
 
