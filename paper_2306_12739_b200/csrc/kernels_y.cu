@@ -323,7 +323,8 @@ k_ypair(DnsDev d, const __grid_constant__ CUtensorMap tmN, const __grid_constant
     double accS[NT][2], accD[NT][2];
     if (!derive_only) {
         // ---- A (element-wise, in place): natural rows (ia, J ia) -> parity rows; H = i kx Nu + i kz Nw -> P0,
-        //      G = i kz Nu - i kx Nw (Eq. 5), RK3 combination, 2 eta_t - h dt Gc -> P1, Nv -> P2, 2 v_t -> P3, eta_t -> P4
+        //      G = i kz Nu - i kx Nw (Eq. 5), RK3 combination, 2 eta_t - h dt Gc -> P1, 2 v_t -> P3; (u.grad)v (P2) and
+        //      eta_t (P4) stay in natural rows for the epilogues of B and C, which own them element by element
 #pragma unroll
         for (int k = 0; k < NT; ++k) {
             const int q = threadIdx.x + k * blockDim.x, ia = q / ET, e = q - ia * ET;
@@ -332,7 +333,7 @@ k_ypair(DnsDev d, const __grid_constant__ CUtensorMap tmN, const __grid_constant
             double* a0 = P0 + ia * ld + 2 * e;
             double* b0 = P0 + ib * ld + 2 * e;
             const double2 nuA = ld2(a0), nuB = ld2(b0), nwA = ld2(a0 + PS), nwB = ld2(b0 + PS);
-            const double2 nvA = ld2(a0 + 2 * PS), nvB = ld2(b0 + 2 * PS), vtA = ld2(a0 + 3 * PS), vtB = ld2(b0 + 3 * PS);
+            const double2 vtA = ld2(a0 + 3 * PS), vtB = ld2(b0 + 3 * PS);
             const double2 etA = ld2(a0 + 4 * PS), etB = ld2(b0 + 4 * PS);
             const double2 HA = make_double2(-kx * nuA.y - kz * nwA.y, kx * nuA.x + kz * nwA.x);
             const double2 HB = make_double2(-kx * nuB.y - kz * nwB.y, kx * nuB.x + kz * nwB.x);
@@ -359,15 +360,11 @@ k_ypair(DnsDev d, const __grid_constant__ CUtensorMap tmN, const __grid_constant
             const double2 rB = make_double2(2.0 * etB.x - hdt * GcB.x, 2.0 * etB.y - hdt * GcB.y);
             st2(a0, make_double2(HA.x + HB.x, HA.y + HB.y));
             st2(a0 + PS, make_double2(rA.x + rB.x, rA.y + rB.y));
-            st2(a0 + 2 * PS, make_double2(nvA.x + nvB.x, nvA.y + nvB.y));
             st2(a0 + 3 * PS, make_double2(2.0 * (vtA.x + vtB.x), 2.0 * (vtA.y + vtB.y)));
-            st2(a0 + 4 * PS, make_double2(etA.x + etB.x, etA.y + etB.y));
             if (ib != ia) {
                 st2(b0, make_double2(HA.x - HB.x, HA.y - HB.y));
                 st2(b0 + PS, make_double2(rA.x - rB.x, rA.y - rB.y));
-                st2(b0 + 2 * PS, make_double2(nvA.x - nvB.x, nvA.y - nvB.y));
                 st2(b0 + 3 * PS, make_double2(2.0 * (vtA.x - vtB.x), 2.0 * (vtA.y - vtB.y)));
-                st2(b0 + 4 * PS, make_double2(etA.x - etB.x, etA.y - etB.y));
             }
         }
         __syncthreads();
@@ -377,8 +374,12 @@ k_ypair(DnsDev d, const __grid_constant__ CUtensorMap tmN, const __grid_constant
 #pragma unroll
         for (int nt = 0; nt < NT; ++nt) {
             double2 FS = make_double2(0.0, 0.0), FD = make_double2(0.0, 0.0);
-            if (sok) { const double2 nv = ld2(P2 + offS + 8 * nt); FS = make_double2(-alpha * nv.x - accS[nt][0], -alpha * nv.y - accS[nt][1]); }
-            if (dok) { const double2 nv = ld2(P2 + offD + 8 * nt); FD = make_double2(-alpha * nv.x - accD[nt][0], -alpha * nv.y - accD[nt][1]); }
+            // (u.grad)v is still in natural rows (i at offS, J i at offD): its parity parts are formed here, in registers
+            if (sok) {
+                const double2 na = ld2(P2 + offS + 8 * nt), nb = dok ? ld2(P2 + offD + 8 * nt) : na;
+                FS = make_double2(-alpha * (na.x + nb.x) - accS[nt][0], -alpha * (na.y + nb.y) - accS[nt][1]);
+                if (dok) FD = make_double2(-alpha * (na.x - nb.x) - accD[nt][0], -alpha * (na.y - nb.y) - accD[nt][1]);
+            }
             // natural rows: F(i) = (FS + FD)/2, F(Ji) = (FS - FD)/2
             const double2 FA = make_double2(0.5 * (FS.x + FD.x), 0.5 * (FS.y + FD.y));
             const double2 FB = make_double2(0.5 * (FS.x - FD.x), 0.5 * (FS.y - FD.y));
@@ -412,17 +413,20 @@ k_ypair(DnsDev d, const __grid_constant__ CUtensorMap tmN, const __grid_constant
 #pragma unroll
         for (int nt = 0; nt < NT; ++nt) {
             double2 vS = make_double2(0.0, 0.0), vD = vS, eS = vS, eD = vS;
+            // eta_t is still in natural rows (i at offS, J i at offD); eta' replaces it in parity form
+            double2 ea = make_double2(0.0, 0.0), eb = ea;
+            if (sok) { ea = ld2(P4 + offS + 8 * nt); eb = dok ? ld2(P4 + offD + 8 * nt) : ea; }
             if (sok) {
-                const double2 v2 = ld2(P3 + offS + 8 * nt), et = ld2(P4 + offS + 8 * nt);
+                const double2 v2 = ld2(P3 + offS + 8 * nt);
                 vS = make_double2(accS[nt][0] - 0.5 * v2.x, accS[nt][1] - 0.5 * v2.y);
-                eS = make_double2(acc2S[nt][0] - et.x, acc2S[nt][1] - et.y);
+                eS = make_double2(acc2S[nt][0] - (ea.x + eb.x), acc2S[nt][1] - (ea.y + eb.y));
                 st2(P0 + offS + 8 * nt, vS);
                 st2(P4 + offS + 8 * nt, eS);
             }
             if (dok) {
-                const double2 v2 = ld2(P3 + offD + 8 * nt), et = ld2(P4 + offD + 8 * nt);
+                const double2 v2 = ld2(P3 + offD + 8 * nt);
                 vD = make_double2(accD[nt][0] - 0.5 * v2.x, accD[nt][1] - 0.5 * v2.y);
-                eD = make_double2(acc2D[nt][0] - et.x, acc2D[nt][1] - et.y);
+                eD = make_double2(acc2D[nt][0] - (ea.x - eb.x), acc2D[nt][1] - (ea.y - eb.y));
                 st2(P0 + offD + 8 * nt, vD);
                 st2(P4 + offD + 8 * nt, eD);
             }
