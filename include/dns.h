@@ -114,6 +114,19 @@ int dns_get_state(dns_plan* plan, double* vhat, double* etahat, double* U00, dou
  * Returns DNS_ENONFINITE if any member's energy is not finite (rows are still filled). */
 int dns_diagnostics(dns_plan* plan, double* out);
 
+/* One-point statistics: running sums, per member and wall-normal point, of
+ * U (plane-mean streamwise velocity), <u'u'>, <v'v'>, <w'w'>, <u'v'> (primes = deviations from the (x,z) plane mean),
+ * evaluated from the spectral state by Parseval over the retained modes.
+ *   dns_stats_reset      -- zero the sums and the sample count (also done by dns_plan_bind)
+ *   dns_stats_accumulate -- enqueue: add the statistics of the current state as one sample
+ *   dns_stats_get        -- out[E][Ny][5] (host or device) = sums / samples; *nsamples (may be NULL) = sample count;
+ *                           synchronises.  With no sample yet out is zero-filled.
+ * Errors: DNS_EINVAL (null), DNS_ESTATE (no workspace / no state), DNS_ECUDA. */
+enum { DNS_NSTAT = 5 };
+int dns_stats_reset(dns_plan* plan);
+int dns_stats_accumulate(dns_plan* plan);
+int dns_stats_get(dns_plan* plan, double* out, long long* nsamples);
+
 /* dns_debug_fetch -- test hook: copy one INTERNAL device array to a host buffer, synchronising first.  Internal
  * spectral layout is [Ny][nkx][nkz][E] complex128 (member index fastest).  which: 0 u, 1 w, 2 du/dy, 3 dw/dy
  * (current stage, Eq. 17-18), 4 the three spectral advection terms (u.grad)u,(u.grad)v,(u.grad)w back to back,

@@ -16,7 +16,8 @@ fourth derivative; P4 divergence / vorticity identities and exact no-slip; P5 fl
 closed-form Crank-Nicolson amplification of a Squire mode; P7 Orr-Sommerfeld growth rate and phase speed
 against an independent generalised eigen-solve and Orszag's published eigenvalue; P8 temporal order;
 P9 the dealiasing cut-off; P10 translation / reflection covariance; P11 the kinetic-energy budget;
-P12 member independence; P13 LU path vs explicitly inverted matrices; P14 single-harmonic DFT.
+P12 member independence; P13 LU path vs explicitly inverted matrices; P14 single-harmonic DFT;
+P15 one-point statistics against Parseval sums and the closed form of a single spanwise mode.
 Parity with the author's MATLAB output: UNPINNED (code and data are not available here); in particular
 reading A7 (only d^4/dy^4 uses the clamped matrix) is pinned against the PDE, not against that code.
 
@@ -316,6 +317,24 @@ class Oracle:
         dens = np.abs(u) ** 2 + np.abs(v0) ** 2 + np.abs(w) ** 2         # [E][nkx][nkz][Ny]
         cn = np.where(self.n_of == 0, 1.0, 2.0)[None, :, None, None]
         return 0.25 * np.einsum("enmj,j->e", cn * dens, self.w)
+
+    def one_point_stats(self):
+        """One-point statistics of the current state ("the time-averaged streamwise- and
+        spanwise-mean velocity profile U(y), the rms profile of the velocity fluctuations from the mean profile
+        (u', v', w') and the tangential Reynolds stress u'v'"): for one instant, the plane averages over the
+        padded physical grid, written out as the definition -- [E][Ny][5] = U, <u'u'>, <v'v'>, <w'w'>, <u'v'>,
+        primes = deviations from the (x, z) plane mean.  A time average is the mean of these over samples."""
+        u, v, w, _, _, _ = self.velocities(self.v, self.eta, self.U, self.W)
+        up, vp, wp = self.to_physical(u), self.to_physical(v), self.to_physical(w)      # [E][Ny][Mx][Mz]
+        out = np.zeros((self.E, self.Ny, 5))
+        Um, Vm, Wm = up.mean(axis=(2, 3)), vp.mean(axis=(2, 3)), wp.mean(axis=(2, 3))
+        uf, vf, wf = up - Um[:, :, None, None], vp - Vm[:, :, None, None], wp - Wm[:, :, None, None]
+        out[:, :, 0] = Um
+        out[:, :, 1] = (uf * uf).mean(axis=(2, 3))
+        out[:, :, 2] = (vf * vf).mean(axis=(2, 3))
+        out[:, :, 3] = (wf * wf).mean(axis=(2, 3))
+        out[:, :, 4] = (uf * vf).mean(axis=(2, 3))
+        return out
 
     def diagnostics(self):
         out = np.zeros((self.E, 6))

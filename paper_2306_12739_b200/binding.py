@@ -22,7 +22,8 @@ _LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libdns_b20
 _lib = None
 
 EXPORTS = ("dns_plan_create", "dns_plan_workspace_bytes", "dns_plan_bind", "dns_set_state", "dns_step",
-           "dns_step_profile", "dns_get_state", "dns_diagnostics", "dns_debug_fetch", "dns_debug_stage", "dns_launches_per_step",
+           "dns_step_profile", "dns_get_state", "dns_diagnostics", "dns_stats_reset", "dns_stats_accumulate", "dns_stats_get",
+           "dns_debug_fetch", "dns_debug_stage", "dns_launches_per_step",
            "dns_plan_destroy",
            "dns_strerror")
 
@@ -60,6 +61,12 @@ def lib():
         L.dns_diagnostics.restype = i
         L.dns_debug_fetch.argtypes = [vp, i, vp, ctypes.c_size_t]
         L.dns_debug_fetch.restype = i
+        L.dns_stats_reset.argtypes = [vp]
+        L.dns_stats_reset.restype = i
+        L.dns_stats_accumulate.argtypes = [vp]
+        L.dns_stats_accumulate.restype = i
+        L.dns_stats_get.argtypes = [vp, dp, ctypes.POINTER(ctypes.c_longlong)]
+        L.dns_stats_get.restype = i
         L.dns_debug_stage.argtypes = [vp, i]
         L.dns_debug_stage.restype = i
         L.dns_launches_per_step.argtypes = [vp]
@@ -123,6 +130,20 @@ def dns_diagnostics(h, out) -> int:
 
 def dns_debug_fetch(h, which: int, out: np.ndarray) -> int:
     return lib().dns_debug_fetch(h, int(which), _ptr(out), ctypes.c_size_t(out.nbytes))
+
+
+def dns_stats_reset(h) -> int:
+    return lib().dns_stats_reset(h)
+
+
+def dns_stats_accumulate(h) -> int:
+    return lib().dns_stats_accumulate(h)
+
+
+def dns_stats_get(h, out: np.ndarray):
+    n = ctypes.c_longlong(0)
+    st = lib().dns_stats_get(h, _ptr(out), ctypes.byref(n))
+    return st, int(n.value)
 
 
 def dns_debug_stage(h, stage: int) -> int:
@@ -211,6 +232,19 @@ class Plan:
         self._chk(dns_debug_fetch(self.h, which, out), "dns_debug_fetch")
         out = np.ascontiguousarray(out.transpose(0, 4, 2, 3, 1))
         return out if nf > 1 else out[0]
+
+    def stats_reset(self):
+        self._chk(dns_stats_reset(self.h), "dns_stats_reset")
+
+    def stats_accumulate(self):
+        self._chk(dns_stats_accumulate(self.h), "dns_stats_accumulate")
+
+    def stats(self):
+        """(mean one-point statistics [E][Ny][5] = U, <u'u'>, <v'v'>, <w'w'>, <u'v'>; number of samples)"""
+        out = np.empty((self.E, self.Ny, 5))
+        st, n = dns_stats_get(self.h, out)
+        self._chk(st, "dns_stats_get")
+        return out, n
 
     def debug_stage(self, stage):
         self._chk(dns_debug_stage(self.h, stage), "dns_debug_stage")

@@ -47,6 +47,7 @@ size_t carve_workspace(dns_plan* p, void* base) {
     d.Ut = c.take<double>(NE);  d.Wt = c.take<double>(NE);  d.Us = c.take<double>(NE);  d.Ws = c.take<double>(NE);
     d.gamma = c.take<double>(d.E);  d.Qstar = c.take<double>(d.E);
     d.diag = c.take<double>((size_t)d.E * 6 + NE);
+    d.stat = c.take<double>((size_t)DNS_NSTAT * NE);
     d.stage_io = c.take<double2>(2 * S + 2 * NE);
     return c.off;
 }
@@ -208,6 +209,7 @@ int dns_plan_bind(dns_plan* p, void* ws, size_t bytes, void* stream) {
     if (st != DNS_OK) { p->sticky = st; return st; }
     p->bound = true;
     p->has_state = false;
+    p->nstat = 0;
     return cuda_status(p, cudaMemsetAsync(ws, 0, p->workspace_bytes, p->stream));
 }
 
@@ -323,6 +325,44 @@ int dns_diagnostics(dns_plan* p, double* out) {
     for (int i = 0; i < d.E; ++i)
         if (!std::isfinite(h[(size_t)i * 6])) return DNS_ENONFINITE;
     return DNS_OK;
+}
+
+int dns_stats_reset(dns_plan* p) {
+    if (!p) return DNS_EINVAL;
+    if (p->sticky != DNS_OK) return p->sticky;
+    if (!p->bound) return DNS_ESTATE;
+    p->nstat = 0;
+    return cuda_status(p, cudaMemsetAsync(p->d.stat, 0, (size_t)DNS_NSTAT * p->d.Ny * p->d.E * sizeof(double), p->stream));
+}
+
+int dns_stats_accumulate(dns_plan* p) {
+    if (!p) return DNS_EINVAL;
+    if (p->sticky != DNS_OK) return p->sticky;
+    if (!p->bound || !p->has_state) return DNS_ESTATE;
+    launch_stats(p);
+    ++p->nstat;
+    return cuda_status(p, cudaGetLastError());
+}
+
+int dns_stats_get(dns_plan* p, double* out, long long* nsamples) {
+    if (!p || !out) return DNS_EINVAL;
+    if (p->sticky != DNS_OK) return p->sticky;
+    if (!p->bound) return DNS_ESTATE;
+    const DnsDev& d = p->d;
+    const size_t NE = (size_t)d.Ny * d.E;
+    std::vector<double> h((size_t)DNS_NSTAT * NE), t((size_t)DNS_NSTAT * NE, 0.0);
+    cudaError_t e = cudaMemcpyAsync(h.data(), d.stat, h.size() * sizeof(double), cudaMemcpyDeviceToHost, p->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(p->stream);
+    if (e != cudaSuccess) return cuda_status(p, e);
+    if (p->nstat > 0) {
+        const double inv = 1.0 / (double)p->nstat;
+        for (int k = 0; k < DNS_NSTAT; ++k)
+            for (int j = 0; j < d.Ny; ++j)
+                for (int m = 0; m < d.E; ++m) t[((size_t)m * d.Ny + j) * DNS_NSTAT + k] = h[(size_t)k * NE + (size_t)j * d.E + m] * inv;
+    }
+    e = cudaMemcpy(out, t.data(), t.size() * sizeof(double), is_device_ptr(out) ? cudaMemcpyHostToDevice : cudaMemcpyHostToHost);
+    if (nsamples) *nsamples = p->nstat;
+    return cuda_status(p, e);
 }
 
 int dns_debug_fetch(dns_plan* p, int which, void* dst, size_t nbytes) {

@@ -42,6 +42,7 @@ struct DnsDev {
     double *Ut, *Wt, *Us, *Ws;      // mean profiles at t and at the current stage
     double *gamma, *Qstar; // [E]
     double* diag;          // [E][6] + scratch [Ny][E]
+    double* stat;          // [DNS_NSTAT][Ny][E] running sums of the one-point statistics
     double2* stage_io;     // staging for ABI-layout copies: 2 spectral fields
     size_t S;              // Ny*P*E
     size_t Isz;            // Ny*Mz*ntl*nkx*2^etl
@@ -76,6 +77,7 @@ struct dns_plan {
     int graph_state = 0;
     int sticky = DNS_OK;
     long long nsteps_done = 0;
+    long long nstat = 0;                       // samples in d.stat
     cudaEvent_t ev[2 * 16] = {};
     bool ev_init = false;
 };
@@ -99,3 +101,4 @@ void launch_mean_in(dns_plan* p, const double* U_abi, const double* W_abi);
 void launch_mean_out(dns_plan* p, double* U_abi, double* W_abi);
 void launch_normalise_state(dns_plan* p);
 void launch_diag(dns_plan* p, double t);
+void launch_stats(dns_plan* p);

@@ -623,6 +623,30 @@ __global__ void k_diag_rows(DnsDev d, const double* __restrict__ part, double t)
     o[0] = en; o[1] = dlo; o[2] = dhi; o[3] = 0.5 * q; o[4] = d.gamma[e]; o[5] = t;
 }
 
+// one-point statistics of the current state (row f4): Parseval sums over the retained modes, added to the running sums
+__global__ void k_stats(DnsDev d) {
+    const int j = blockIdx.x;
+    const size_t NE = (size_t)d.Ny * d.E;
+    for (int e = threadIdx.x; e < d.E; e += blockDim.x) {
+        double suu = 0.0, svv = 0.0, sww = 0.0, suv = 0.0;
+        for (int p = 1; p < d.P; ++p) {
+            const size_t gi = ((size_t)j * d.P + p) * d.E + e;
+            const double2 u = d.uh[gi], v = d.vt[gi], w = d.wh[gi];
+            const double cn = (p / d.nkz) == 0 ? 1.0 : 2.0;      // the n = 0 plane stores both +-m, n > 0 stands for +-n
+            suu += cn * (u.x * u.x + u.y * u.y);
+            svv += cn * (v.x * v.x + v.y * v.y);
+            sww += cn * (w.x * w.x + w.y * w.y);
+            suv += cn * (u.x * v.x + u.y * v.y);
+        }
+        const size_t o = (size_t)j * d.E + e;
+        d.stat[o] += d.Ut[o];
+        d.stat[NE + o] += suu;
+        d.stat[2 * NE + o] += svv;
+        d.stat[3 * NE + o] += sww;
+        d.stat[4 * NE + o] += suv;
+    }
+}
+
 }  // namespace
 
 size_t dns_ypair_smem(int Ni, int Ny, int ET) {
@@ -715,6 +739,7 @@ void launch_mean_in(dns_plan* p, const double* U, const double* W) {
 void launch_mean_out(dns_plan* p, double* U, double* W) {
     k_mean_out<<<(p->d.E + 127) / 128, 128, 0, p->stream>>>(p->d, U, W);
 }
+void launch_stats(dns_plan* p) { k_stats<<<p->d.Ny, 128, 0, p->stream>>>(p->d); }
 void launch_diag(dns_plan* p, double t) {
     const DnsDev& d = p->d;
     double* part = d.diag + (size_t)d.E * 6;

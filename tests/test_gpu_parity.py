@@ -307,3 +307,32 @@ def test_stage_pieces_against_oracle():
     assert field_err(plan.debug_fetch(5)[..., 1:-1], F) < 1e-11
     assert field_err(plan.debug_fetch(6)[..., 1:-1], G) < 1e-11
     plan.close()
+
+
+def test_one_point_statistics_against_oracle():
+    """Row f4: running one-point statistics (Parseval sums on the GPU) against the oracle's plane averages on the
+    padded physical grid, accumulated over the same three samples; reset and sample count."""
+    cfg = inputs.CONFIGS[2].with_E(5)
+    st = inputs.make_state(cfg)
+    plan = binding.Plan(*inputs.plan_args(cfg))
+    plan.set_state(st["vhat"], st["etahat"], st["U00"], st["W00"])
+    o = Oracle(*inputs.plan_args(cfg))
+    o.set_state(st["vhat"], st["etahat"], st["U00"], st["W00"])
+    s0, n0 = plan.stats()
+    assert n0 == 0 and np.all(s0 == 0.0)
+    acc = np.zeros((cfg.E, cfg.Ny, 5))
+    for _ in range(3):
+        plan.step(2)
+        o.step(2)
+        plan.stats_accumulate()
+        acc += o.one_point_stats()
+    s, n = plan.stats()
+    assert n == 3
+    ref = acc / 3
+    for k in range(5):
+        scale = max(np.abs(ref[:, :, k]).max(), 1e-300)
+        assert np.abs(s[:, :, k] - ref[:, :, k]).max() < 1e-10 * max(scale, np.abs(ref[:, :, 1]).max()), k
+    plan.stats_reset()
+    s1, n1 = plan.stats()
+    assert n1 == 0 and np.all(s1 == 0.0)
+    plan.close()

@@ -486,3 +486,41 @@ def test_generator_energy_closed_form_matches_oracle_energy():
         lam.set_state(z, z, st["U00"], st["W00"])
         rms = np.sqrt(2 * (o.energy() - lam.energy()))
         assert np.abs(rms - st["rms"]).max() < 1e-9
+
+
+# ------------------------------------------------------------------------------------------------ P15 (row f4)
+def test_P15_one_point_stats_closed_form_single_spanwise_mode():
+    """v = 0 and one vorticity mode eta_hat(n=0, m) = b g(y): Eq. 17-18 give u_hat = -i eta_hat / kz, w = 0, i.e.
+    u'(y, z) = 2 Re(u_hat e^{i kz z}) and <u'u'> = 2 |u_hat|^2, all other second moments zero, U = U00."""
+    cfg = small_cfg(COUETTE, E=1)
+    o = Oracle(*inputs.plan_args(cfg))
+    v = np.zeros((1, o.nkx, o.nkz, o.Ny), np.complex128)
+    eta = np.zeros_like(v)
+    m = 2
+    mi = int(np.where(o.m_of == m)[0][0])
+    g = (1 - o.y ** 2) * (0.3 + 0.5 * o.y)
+    b = 0.7 - 0.4j
+    eta[0, 0, mi, :] = b * g
+    o.set_state(v, eta, o.y[None, :].copy(), np.zeros((1, o.Ny)))
+    s = o.one_point_stats()
+    kz = 2 * PI * m / cfg.Lz
+    assert np.abs(s[0, :, 0] - o.y).max() < 1e-14
+    assert np.abs(s[0, :, 1] - 2 * np.abs(b * g / kz) ** 2).max() < 1e-13
+    assert np.abs(s[0, :, 2:]).max() < 1e-14
+
+
+def test_P15_one_point_stats_match_parseval_sums():
+    """Plane averages on the padded grid (the oracle's route) against the Parseval sums over the Hermitian-completed
+    retained modes (an independent route: no transform involved)."""
+    cfg = small_cfg(POISEUILLE_CMF, E=2, cid=3)
+    o, _ = make(cfg)
+    o.step(2)
+    s = o.one_point_stats()
+    u, v, w, _, _, _ = o.velocities(o.v, o.eta, o.U, o.W)
+    cn = np.where(o.n_of == 0, 1.0, 2.0)[None, :, None, None]
+    mask = np.ones((1, o.nkx, o.nkz, 1))
+    mask[0, 0, 0, 0] = 0.0                                   # the plane mean is not a fluctuation
+    for k, (a, b2) in enumerate(((u, u), (v, v), (w, w), (u, v)), start=1):
+        ref = np.einsum("enmj->ej", cn * mask * (a * np.conj(b2)).real)
+        assert np.abs(s[:, :, k] - ref).max() < 1e-13 * max(1.0, np.abs(ref).max()), k
+    assert np.abs(s[:, :, 0] - o.U).max() < 1e-13
