@@ -719,6 +719,7 @@ void launch_ypair(dns_plan* p, int stage, int derive_only) {
 void launch_mean(dns_plan* p, int stage, int derive_only, cudaStream_t stream) {
     const DnsDev& d = p->d;
     const size_t smem = (size_t)6 * d.Ny * 8 * sizeof(double);
+    if (smem > 48 * 1024) cudaFuncSetAttribute(k_mean, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);   // Ny >= 129
     k_mean<<<(d.E + 7) / 8, 256, smem, stream>>>(d, stage, derive_only);
 }
 

@@ -113,7 +113,8 @@ def test_ragged_member_tiles_of_the_wide_layouts(Nx, Nz, E):
     assert_errs(errs, 2, TOL_1 * 10)
 
 
-@pytest.mark.parametrize("E,Ny,flow", [(1, 17, 0), (5, 20, 1), (33, 12, 0), (7, 5, 1), (2, 66, 1), (6, 75, 0)])
+@pytest.mark.parametrize("E,Ny,flow", [(1, 17, 0), (5, 20, 1), (33, 12, 0), (7, 5, 1), (2, 66, 1), (6, 75, 0),
+                                       (3, 129, 0), (2, 257, 1)])       # 257 = the largest Ny dns_plan_create accepts
 def test_ragged_members_and_odd_even_ny(E, Ny, flow):
     cfg = inputs.Config(3 if flow else 1, flow, 500.0, 2 * PI, PI, 16, Ny, 12, E, 0.01, 1, 0.1, 0, box=2)
     errs, _, _ = run_pair(cfg, range(E), 3, check_at=(1, 3))
