@@ -102,6 +102,26 @@ def test_every_transform_length_both_directions(Nx, Nz):
     assert_errs(errs, 2, TOL_1 * 10)
 
 
+@pytest.mark.parametrize("Nx", [12, 16, 18, 24, 36, 54, 72])
+def test_sixteen_lane_line_kernel_for_every_x_length(Nx):
+    """Every padded x length with an ensemble large enough for the 16-lane member tiles (E = 17: one full tile and a
+    ragged one); oracle on the first and the last member."""
+    cfg = inputs.Config(1, inputs.COUETTE, 350.0, 1.9 * PI, 1.1 * PI, Nx, 13, 16, 17, 0.01, 1, 0.1, 0, box=3)
+    errs, _, _ = run_pair(cfg, [0, 16], 2, check_at=(1, 2))
+    assert_errs(errs, 1, TOL_1)
+    assert_errs(errs, 2, TOL_1 * 10)
+
+
+@pytest.mark.parametrize("Nz", [12, 16, 18, 24, 32, 36, 48, 54, 64, 72])
+def test_every_z_length_with_sixteen_member_tiles(Nz):
+    """Every padded z length (register z transforms for Mz = 24, 36, 48, 72, 96, shared-memory ones otherwise) against
+    the 16-member tiles of the mixed layout, ragged last tile (E = 17)."""
+    cfg = inputs.Config(1, inputs.COUETTE, 350.0, 1.9 * PI, 1.1 * PI, 16, 13, Nz, 17, 0.01, 1, 0.1, 0, box=3)
+    errs, _, _ = run_pair(cfg, [0, 16], 2, check_at=(1, 2))
+    assert_errs(errs, 1, TOL_1)
+    assert_errs(errs, 2, TOL_1 * 10)
+
+
 @pytest.mark.parametrize("Nx,Nz,E", [(48, 32, 17), (32, 48, 9), (32, 32, 21), (64, 16, 19)])
 def test_ragged_member_tiles_of_the_wide_layouts(Nx, Nz, E):
     """Member tiles of 8 and 16 lanes (line kernel, mixed layout) and the two-thread register z transforms with a
