@@ -357,3 +357,29 @@ def test_one_point_statistics_against_oracle():
     s1, n1 = plan.stats()
     assert n1 == 0 and np.all(s1 == 0.0)
     plan.close()
+
+
+def test_rebinding_the_workspace_rebuilds_graph_and_tensor_maps():
+    """dns_plan_bind on a second buffer after steps have been taken: the captured step graph and the TMA descriptors
+    hold pointers into the first buffer and must be rebuilt; results equal those of the first run bit for bit."""
+    import torch
+    cfg = inputs.CONFIGS[2].with_E(6)
+    st = inputs.make_state(cfg)
+    plan = binding.Plan(*inputs.plan_args(cfg))
+    plan.set_state(st["vhat"], st["etahat"], st["U00"], st["W00"])
+    plan.step(2)
+    first = plan.get_state()
+    n = plan.workspace_bytes
+    ws2 = torch.empty(n + 256, dtype=torch.uint8, device="cuda")
+    base = (ws2.data_ptr() + 255) & ~255
+    assert binding.dns_plan_bind(plan.h, base, n) == binding.DNS_OK
+    assert binding.dns_step(plan.h, 1) == binding.DNS_ESTATE                 # the state went with the old workspace
+    plan.workspace.fill_(0xFF)                                               # poison the old buffer
+    plan.set_state(st["vhat"], st["etahat"], st["U00"], st["W00"])
+    plan.step(1)
+    plan.step(1)
+    second = plan.get_state()
+    for a, b in zip(first, second):
+        assert np.array_equal(a, b)
+    plan.close()
+    del ws2
