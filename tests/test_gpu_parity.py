@@ -383,3 +383,24 @@ def test_rebinding_the_workspace_rebuilds_graph_and_tensor_maps():
         assert np.array_equal(a, b)
     plan.close()
     del ws2
+
+
+def test_plan_on_a_non_default_stream():
+    """The plan works on whatever stream it is bound to (here a torch side stream): graph replay, the internal
+    mean-flow stream and the copies are all ordered on it; same bits as on the default stream."""
+    import torch
+    cfg = inputs.CONFIGS[2].with_E(6)
+    st = inputs.make_state(cfg)
+    outs = []
+    for use_side in (False, True):
+        s = torch.cuda.Stream() if use_side else torch.cuda.current_stream()
+        with torch.cuda.stream(s):
+            plan = binding.Plan(*inputs.plan_args(cfg))
+            plan.set_state(st["vhat"], st["etahat"], st["U00"], st["W00"])
+            plan.step(3)
+            outs.append(plan.get_state())
+            d = plan.diagnostics()
+            assert np.all(np.isfinite(d))
+            plan.close()
+    for a, b in zip(*outs):
+        assert np.array_equal(a, b)
