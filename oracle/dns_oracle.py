@@ -17,7 +17,9 @@ closed-form Crank-Nicolson amplification of a Squire mode; P7 Orr-Sommerfeld gro
 against an independent generalised eigen-solve and Orszag's published eigenvalue; P8 temporal order;
 P9 the dealiasing cut-off; P10 translation / reflection covariance; P11 the kinetic-energy budget;
 P12 member independence; P13 LU path vs explicitly inverted matrices; P14 single-harmonic DFT;
-P15 one-point statistics against Parseval sums and the closed form of a single spanwise mode.
+P15 one-point statistics against Parseval sums and the closed form of a single spanwise mode;
+P16 the RK3 stage weights of PAPER.md:126 against Kutta's amplification polynomial 1 + z + z^2/2 + z^3/6 of an
+inviscid pointwise-advection Squire mode (and third-order convergence in that limit).
 Parity with the author's MATLAB output: UNPINNED (code and data are not available here); in particular
 reading A7 (only d^4/dy^4 uses the clamped matrix) is pinned against the PDE, not against that code.
 

@@ -331,6 +331,80 @@ def test_P8_temporal_order_two():
     assert 3.3 < r1 < 5.0 and 3.3 < r2 < 5.2, (errs, r1, r2)
 
 
+# ------------------------------------------------------------------------------------------------ P16
+def _inviscid_squire_step(dt, Re=1e12, Ny=25, n=2, step=None):
+    """One step of a Squire mode (v = 0, kz = 0, eta = 1e-9 g(y)) on the parabola U = 1 - y^2 at Re -> infinity.
+    Eq. 17-18 give u = 0, w = i eta/kx, hence G = i kx U(y) eta (Eq. 5) and every collocation point is its own
+    eigenmode d eta_j/dt = lambda_j eta_j, lambda_j = -i kx U(y_j).  Returns (eta_0, eta_1, z_j = lambda_j dt)."""
+    Lx = 2 * PI
+    o = Oracle(12, Ny, 12, 1, Re, Lx, PI, dt, POISEUILLE_CMF)
+    if step is not None:
+        o.step = step.__get__(o)
+    g = (1 - o.y ** 2) * (1 + 0.3 * o.y) * np.exp(0.7j * o.y)
+    vh = np.zeros((1, 6, 11, Ny), complex)
+    eh = np.zeros_like(vh)
+    eh[0, n, 0] = 1e-9 * g
+    o.set_state(vh, eh, (1 - o.y ** 2)[None], np.zeros((1, Ny)))
+    e0 = o.eta[0, n, 0].copy()
+    o.step(1)
+    kx = 2 * PI * n / Lx
+    assert np.abs(o.v).max() < 1e-16 and np.abs(o.U[0] - (1 - o.y ** 2)).max() < 1e-12
+    return e0, o.eta[0, n, 0].copy(), -1j * kx * (1 - o.y ** 2) * dt
+
+
+def test_P16_rk3_weights_kutta_amplification_polynomial():
+    """PAPER.md:126 (F^0 with h = 1/2; 2 F^1 - F^0 with h = 1; (F^0 + 4 F^1 + F^2)/6 with h = 1) is Kutta's
+    third-order scheme: on d eta/dt = lambda eta with the Crank-Nicolson part switched off (Re = 1e12) one step
+    multiplies eta by EXACTLY 1 + z + z^2/2 + z^3/6, z = lambda dt.  With kx dt = 0.3 the cubic term is 4.5e-3, so
+    a wrong stage weight is visible at 1e-3 against a tolerance of 1e-10 (the oracle itself: 1.0e-12).  Mutations
+    of Oracle.step that pass every other pin (P2, P7, P8, P10, P11; round-1 review) and their error here, measured
+    while writing this pin: stage 2 <- F^1 2.2e-3, stage 3 <- (F^0 + 2 F^1 + F^2)/4 2.2e-3, stage 3 <- F^1 4.4e-3
+    (test_P16_detects_wrong_rk3_weights keeps them red)."""
+    e0, e1, z = _inviscid_squire_step(dt=0.15)
+    kutta = 1 + z + z ** 2 / 2 + z ** 3 / 6
+    assert np.abs(z ** 3 / 6).max() > 4e-3
+    err = np.abs(e1 - kutta * e0).max() / np.abs(e0).max()
+    assert err < 1e-10, err
+
+
+@pytest.mark.parametrize("mutation", ["stage2_F1", "stage3_quarter", "stage3_F1"])
+def test_P16_detects_wrong_rk3_weights(mutation):
+    """The pin above is discriminating: a copy of Oracle.step with one wrong weighting (the three the round-1 review
+    found invisible to P1-P15) misses the Kutta polynomial by more than 1e-3."""
+    def step(self, nsteps=1):
+        for _ in range(int(nsteps)):
+            s_t = (self.v, self.eta, self.U, self.W)
+            N0 = self.nonlinear(*s_t)
+            s1 = self.stage(*s_t, 0.5, *N0)
+            N1 = self.nonlinear(*s1[:4])
+            c2 = N1 if mutation == "stage2_F1" else tuple(2.0 * a - b for a, b in zip(N1, N0))
+            s2 = self.stage(*s_t, 1.0, *c2)
+            N2 = self.nonlinear(*s2[:4])
+            if mutation == "stage3_quarter":
+                c3 = tuple((a + 2.0 * b + c) / 4.0 for a, b, c in zip(N0, N1, N2))
+            elif mutation == "stage3_F1":
+                c3 = N1
+            else:
+                c3 = tuple((a + 4.0 * b + c) / 6.0 for a, b, c in zip(N0, N1, N2))
+            self.v, self.eta, self.U, self.W, self.gamma = self.stage(*s_t, 1.0, *c3)
+            self.t += self.dt
+
+    e0, e1, z = _inviscid_squire_step(dt=0.15, step=step)
+    kutta = 1 + z + z ** 2 / 2 + z ** 3 / 6
+    assert np.abs(e1 - kutta * e0).max() / np.abs(e0).max() > 1e-3
+
+
+def test_P16_third_order_in_the_advection_dominated_limit():
+    """Second pin of the weights: at Re = 1e9 the error of one inviscid Squire step against exp(z) falls by ~2^4
+    per halving of dt (local error of a third-order scheme), not by 2^3 as a second-order weighting would give."""
+    errs = []
+    for dt in (0.2, 0.1, 0.05):
+        e0, e1, z = _inviscid_squire_step(dt=dt, Re=1e9)
+        errs.append(np.abs(e1 - np.exp(z) * e0).max() / np.abs(e0).max())
+    r1, r2 = errs[0] / errs[1], errs[1] / errs[2]
+    assert 13.0 < r1 < 19.0 and 13.0 < r2 < 19.0, (errs, r1, r2)
+
+
 # ------------------------------------------------------------------------------------------------ P9 / P14
 def test_P14_single_harmonic_dft_roundtrip():
     cfg = small_cfg()
