@@ -96,8 +96,8 @@ int dns_set_state(dns_plan* plan, const double* vhat, const double* etahat, cons
 
 /* dns_step -- enqueue nsteps full CN/RK3 time steps (3 stages each) on the plan's stream
  * and return without synchronising.  The 15 launches of a step are captured once into a CUDA graph (on an internal
- * stream, at the first call after dns_plan_bind) and replayed per step; DNS_GRAPH=0 in the environment, or a failed
- * capture, falls back to direct launches with identical results.  Errors: DNS_EINVAL (nsteps < 0), DNS_ESTATE (no state), DNS_ECUDA. */
+ * stream, at the first call after dns_plan_bind) and replayed per step; a failed capture (or the test option "graph" = 0 of include/dns_debug.h) falls back to
+ * direct launches with identical results.  Errors: DNS_EINVAL (nsteps < 0), DNS_ESTATE (no state), DNS_ECUDA. */
 int dns_step(dns_plan* plan, int nsteps);
 
 /* dns_step_profile -- as dns_step, but brackets every kernel class with CUDA events on the plan's stream,
@@ -126,19 +126,6 @@ enum { DNS_NSTAT = 5 };
 int dns_stats_reset(dns_plan* plan);
 int dns_stats_accumulate(dns_plan* plan);
 int dns_stats_get(dns_plan* plan, double* out, long long* nsamples);
-
-/* dns_debug_fetch -- test hook: copy one INTERNAL device array to a host buffer, synchronising first.  Internal
- * spectral layout is [Ny][nkx][nkz][E] complex128 (member index fastest).  which: 0 u, 1 w, 2 du/dy, 3 dw/dy
- * (current stage, Eq. 17-18), 4 the three spectral advection terms (u.grad)u,(u.grad)v,(u.grad)w back to back,
- * 5 F and 6 G history (Eq. 4-5, interior rows: F^0 after stage 0, F^0 + 4 F^1 after stage 1), 7 v of
- * the current stage, 8 U00 and
- * 9 W00 of the current stage as [Ny][E] float64.  nbytes must equal the array size (DNS_EINVAL otherwise). */
-int dns_debug_fetch(dns_plan* plan, int which, void* host_dst, size_t nbytes);
-
-/* dns_debug_stage -- test hook: enqueue ONE Crank-Nicolson/RK3 stage (0, 1 or 2) on the
- * plan's stream, so that per-stage internals can be fetched.  A step is stages 0, 1, 2 in order; the step
- * counter advances after stage 2.  Errors: DNS_EINVAL (stage outside 0..2), DNS_ESTATE, DNS_ECUDA. */
-int dns_debug_stage(dns_plan* plan, int stage);
 
 /* Number of kernel launches one dns_step(1) enqueues (for bench.py's gpu_launches). */
 int dns_launches_per_step(const dns_plan* plan);

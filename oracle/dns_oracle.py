@@ -20,6 +20,10 @@ P12 member independence; P13 LU path vs explicitly inverted matrices; P14 single
 P15 one-point statistics against Parseval sums and the closed form of a single spanwise mode;
 P16 the RK3 stage weights of PAPER.md:126 against Kutta's amplification polynomial 1 + z + z^2/2 + z^3/6 of an
 inviscid pointwise-advection Squire mode (and third-order convergence in that limit).
+Rows f1 / f2 of SURVEY.md 8(f) (tests/test_oracle_pins_forms.py): P17 the rotational form omega x u against the vector
+identity (u.grad)u = omega x u + grad(|u|^2/2), pointwise orthogonality to u, the Orr-Sommerfeld growth rates, the laminar
+fixed points, the energy budget and the Kutta polynomial; P18 the ensemble-coupled streamwise-mean flow
+against the identical-member limit, the shared-mean invariant and the ensemble-mean energy budget.
 Parity with the author's MATLAB output: UNPINNED (code and data are not available here); in particular
 reading A7 (only d^4/dy^4 uses the clamped matrix) is pinned against the PDE, not against that code.
 
@@ -32,6 +36,10 @@ import scipy.linalg as sla
 
 COUETTE = 0
 POISEUILLE_CMF = 1
+CONVECTIVE = 0        # nonlinear term u . grad u_i, the paper's form
+ROTATIONAL = 1        # omega x u (reading F1 of DESIGN.md)
+UNCOUPLED = 0         # independent members
+STREAMWISE_MEAN = 1   # members share the streamwise-mean flow (row f2, reading F2 of DESIGN.md)
 
 
 # --------------------------------------------------------------------------------------------------
@@ -101,9 +109,10 @@ class Oracle:
     0..Nz/2-1, -(Nz/2-1)..-1, PAPER.md:188), U00, W00 [E][Ny].
     """
 
-    def __init__(self, Nx, Ny, Nz, E, Re, Lx, Lz, dt, flow):
+    def __init__(self, Nx, Ny, Nz, E, Re, Lx, Lz, dt, flow, form=CONVECTIVE, coupling=UNCOUPLED):
         self.Nx, self.Ny, self.Nz, self.E = int(Nx), int(Ny), int(Nz), int(E)
         self.Re, self.Lx, self.Lz, self.dt, self.flow = float(Re), float(Lx), float(Lz), float(dt), int(flow)
+        self.form, self.coupling = int(form), int(coupling)
         self.Mx, self.Mz = 3 * self.Nx // 2, 3 * self.Nz // 2          # 3/2 rule (PAPER.md:182)
         self.nkx, self.nkz = self.Nx // 2, self.Nz - 1                 # retained |n| <= Nx/2-1 (reading A2, A3)
         self.Ni = self.Ny - 2
@@ -185,6 +194,16 @@ class Oracle:
     def get_state(self):
         return self.v.copy(), self.eta.copy(), self.U.copy(), self.W.copy()
 
+    def add_increment(self, dv, deta):
+        """state += (dv, deta) between two steps: how a caller applies one realisation of a stochastic forcing
+        (the realisations themselves are the caller's, reading F2).  Wall rows, the (0,0) column and
+        the m < 0 half of the n = 0 plane of the result are normalised as in set_state."""
+        v = self.v + np.asarray(dv, dtype=np.complex128).reshape(self.v.shape)
+        eta = self.eta + np.asarray(deta, dtype=np.complex128).reshape(self.eta.shape)
+        t, g, Q = self.t, self.gamma, self.Qstar
+        self.set_state(v, eta, self.U, self.W)
+        self.t, self.gamma, self.Qstar = t, g, Q
+
     # ---------------------------------------------------------------- a1-a3: velocities from (v, eta) (Eq. 17-18)
     def velocities(self, v, eta, U, W):
         """u, w (and Dv, Du, Dw) in spectral space; wall rows imposed (reading A10); (0,0) = mean profiles."""
@@ -228,20 +247,52 @@ class Oracle:
         return fh / (self.Mx * self.Mz)
 
     # ---------------------------------------------------------------- O-nonlinear (a1-a7)
-    def nonlinear(self, v, eta, U, W):
-        """F, G at interior rows for all (n,m), S_u = D [uv]00, S_w = D [wv]00 (PAPER.md:72-78 Eq. 4-7, :108,
-        convective form u . grad u_i, reading A11)."""
+    def advection(self, v, eta, U, W):
+        """The nonlinear vector in physical space on the padded grid, real [E][Ny][Mx][Mz] each, and the two mean-flow
+        sources S_u, S_w [E][Ny] of Eq. 6-7.
+        CONVECTIVE (the paper's form): N_i = u . grad u_i; S_u = d/dy [uv]00, S_w = d/dy [wv]00 with the
+        plane means of the products (reading A9).
+        ROTATIONAL (row f1): H = omega x u with omega = curl u = (dw/dy - dv/dz, du/dz - dw/dx, dv/dx - du/dy).
+        Since (u . grad)u = omega x u + grad(|u|^2/2) and Eq. 4-5 are what is left of the momentum equation once
+        gradients are eliminated, F and G keep their form with H in place of N; the plane mean of
+        d/dx(|u|^2/2) vanishes, so the mean-flow sources are the plane means of H_x and H_z themselves."""
         ikx = 1j * self.kx[None, :, None, None]
         ikz = 1j * self.kz[None, None, :, None]
         u, v0, w, Du, Dv, Dw = self.velocities(v, eta, U, W)
         P = self.to_physical
         pu, pv, pw = P(u), P(v0), P(w)
-        Nu = pu * P(ikx * u) + pv * P(Du) + pw * P(ikz * u)            # u . grad u   (a5)
-        Nv = pu * P(ikx * v0) + pv * P(Dv) + pw * P(ikz * v0)          # u . grad v
-        Nw = pu * P(ikx * w) + pv * P(Dw) + pw * P(ikz * w)            # u . grad w
-        uv00 = np.mean(pu * pv, axis=(2, 3))                           # plane means [uv]00(y) (reading A9)
-        wv00 = np.mean(pw * pv, axis=(2, 3))
+        if self.form == CONVECTIVE:
+            Nu = pu * P(ikx * u) + pv * P(Du) + pw * P(ikz * u)            # u . grad u   (a5)
+            Nv = pu * P(ikx * v0) + pv * P(Dv) + pw * P(ikz * v0)          # u . grad v
+            Nw = pu * P(ikx * w) + pv * P(Dw) + pw * P(ikz * w)            # u . grad w
+            uv00 = np.mean(pu * pv, axis=(2, 3))                           # plane means [uv]00(y) (reading A9)
+            wv00 = np.mean(pw * pv, axis=(2, 3))
+            Su = uv00 @ self.D.T                                           # d/dy [uv]00 (Eq. 6)
+            Sw = wv00 @ self.D.T                                           # d/dy [wv]00 (Eq. 7)
+            return Nu, Nv, Nw, Su, Sw
+        ox = P(Dw - ikz * v0)                                              # omega_x = dw/dy - dv/dz
+        oy = P(ikz * u - ikx * w)                                          # omega_y = du/dz - dw/dx (= eta, PAPER.md:68)
+        oz = P(ikx * v0 - Du)                                              # omega_z = dv/dx - du/dy
+        Hx = oy * pw - oz * pv
+        Hy = oz * pu - ox * pw
+        Hz = ox * pv - oy * pu
+        return Hx, Hy, Hz, np.mean(Hx, axis=(2, 3)), np.mean(Hz, axis=(2, 3))
+
+    def nonlinear(self, v, eta, U, W):
+        """F, G at interior rows for all (n,m) and the mean-flow sources S_u, S_w (PAPER.md:72-78 Eq. 4-7, :108).
+        With coupling = STREAMWISE_MEAN (row f2: "Each ensemble member shares a common streamwise
+        mean flow, which is updated at every time-step by the perturbation Reynolds stresses averaged over the
+        ensemble members") the kx = 0 part of the nonlinear vector -- all that forces the streamwise-mean flow -- and
+        the two mean-flow sources are replaced by their average over the members; n != 0 is untouched."""
+        ikx = 1j * self.kx[None, :, None, None]
+        ikz = 1j * self.kz[None, None, :, None]
+        Nu, Nv, Nw, Su, Sw = self.advection(v, eta, U, W)
         Nuh, Nvh, Nwh = self.to_spectral(Nu), self.to_spectral(Nv), self.to_spectral(Nw)   # a6
+        if self.coupling == STREAMWISE_MEAN:
+            for f in (Nuh, Nvh, Nwh):
+                f[:, 0, :, :] = np.sum(f[:, 0, :, :], axis=0) / f.shape[0]
+            Su = np.tile(np.sum(Su, axis=0) / Su.shape[0], (Su.shape[0], 1))
+            Sw = np.tile(np.sum(Sw, axis=0) / Sw.shape[0], (Sw.shape[0], 1))
         al = self.alpha[None, :, :, None]
         F = -al * Nvh - ikx * (Nuh @ self.D.T) - ikz * (Nwh @ self.D.T)   # a7 (Eq. 4 with Eq. 10's sign)
         G = ikz * Nuh - ikx * Nwh                                          # a7 (Eq. 5)
@@ -249,8 +300,6 @@ class Oracle:
         G = G[..., 1:-1].copy()
         F[:, 0, 0, :] = 0.0
         G[:, 0, 0, :] = 0.0
-        Su = uv00 @ self.D.T                                           # d/dy [uv]00 (Eq. 6)
-        Sw = wv00 @ self.D.T                                           # d/dy [wv]00 (Eq. 7)
         return F, G, Su, Sw
 
     # ---------------------------------------------------------------- O-stage (a9, a10)
