@@ -1,15 +1,19 @@
 #!/usr/bin/env python
 """bench.py -- ensemble member-steps/s of the CN/RK3 ensemble DNS step (arXiv 2306.12739) on B200.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--impl reference]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--form convective] [--impl reference]
 
 One "step" = one dns_step(1): the whole hot path (3 RK stages x {z-FFT, fused x-line kernel, z-FFT, per-pair DMMA
-kernel; the mean-flow kernel runs beside the last two on a side stream}: 15 launches) over the whole ensemble.  At N = 1 the workload is BASELINE.json configs[1]
-(plane Couette, Re = 1000, 32 x 49 x 32, E = 64, fp64).  For N > 1 (torchrun, one rank per GPU) every rank advances
-its own 64 members (weak scaling; members are independent, no data-path collective -- SURVEY.md 8(e)).
+kernel; the mean-flow kernel runs beside the last two on a side stream}: 15 launches) over the whole ensemble.  At N = 1
+the workload is BASELINE.json configs[3] (Poiseuille at constant mass flux, 48 x 65 x 48, E = 256, fp64): BASELINE.json's
+metric names no configuration, and this is the largest single-GPU workload of the five (the paper's C1/P1 x-z
+resolution) -- `--config 2` gives configs[1].  For N > 1 (torchrun, one rank per GPU) every rank advances
+its own E members (weak scaling; members are independent, no data-path collective -- SURVEY.md 8(e)).
 Prints ONE JSON line on rank 0 (contract in the task statement): value = whole-job member-steps/s with the state
-resident in HBM; e2e = the same through the C ABI with HOST buffers (H2D + step + D2H every step);
-roofline = the dominant kernel against the measured HBM / fp64 peaks; cpu_baseline = the oracle on the host cores.
+resident in HBM, in the paper's convective form of the nonlinear term; "rotational" = the same
+measurement in the rotational form; e2e = through the C ABI with HOST buffers (H2D + step + D2H
+every step); roofline = the dominant kernel against the measured HBM / fp64 peaks (the fp64 peak is measured live by
+dns_debug_fp64_peak); cpu_baseline = the oracle on the host cores.
 `--impl reference` times the oracle (oracle/dns_oracle.py) alone, as it stands, on a bounded sample.
 """
 from __future__ import annotations
@@ -30,7 +34,7 @@ from paper_2306_12739_b200 import inputs  # noqa: E402
 
 METRIC = "ensemble member-steps/s (fp64, device-timed)"
 UNIT = "member-steps/s"
-FP64_PEAK_TFLOPS = 37.0   # measured on this pool's B200: DMMA.8x8x4 and DFMA both 37.0 TFLOP/s
+FP64_PEAK_FALLBACK = 37.0   # used only if the live microbenchmark fails (148 SMs x 64 FMA/clk x 2 x 1.965 GHz = 37.2)
 
 
 def measured_peaks():
@@ -92,7 +96,7 @@ class ClockSampler(threading.Thread):
         return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
 
 
-def workload_counts(cfg, E):
+def workload_counts(cfg, E, rot=False):
     """Algorithmic bytes / flops per kernel class per STAGE for E members."""
     Ni, P = cfg.Ny - 2, (cfg.Nx // 2) * (cfg.Nz - 1)
     Mx, Mz, nkx, nkz = 3 * cfg.Nx // 2, 3 * cfg.Nz // 2, cfg.Nx // 2, cfg.Nz - 1
@@ -103,6 +107,14 @@ def workload_counts(cfg, E):
     fx = 5.0 * Mx * lg(Mx)
     nmat = nkx * (cfg.Nz // 2) - 1
     Kh, Kho = (Ni + 1) // 2, Ni // 2
+    if rot:   # 6 fields in and out of the z inverse, 6 in + 3 out of the line kernel (3 + 2 transforms), eta' as a 14th field
+        return {
+            "fft_z_inv": {"bytes": 6 * S + 6 * I, "flops": 6 * Ni * nkx * E * fz},
+            "line_fft_x_products": {"bytes": 9 * I + Ni * Mz * E * 16.0, "flops": Ni * Mz * E * (5 * fx + 9.0 * Mx)},
+            "fft_z_fwd": {"bytes": 3 * I + 3 * S, "flops": 3 * Ni * nkx * E * fz},
+            "ypair_dmma": {"bytes": 14 * S + 3 * (Kh * Kh + Kho * Kho) * 8.0 * nmat + Ni * Mz * E * 16.0 + 12 * cfg.Ny * E * 8.0,
+                           "flops": 7 * 2.0 * (Kh * Kh + Kho * Kho) * 2 * E * (P - 1)},
+        }
     return {
         "fft_z_inv": {"bytes": 5 * S + 8 * I, "flops": 8 * Ni * nkx * E * fz},
         "line_fft_x_products": {"bytes": 11 * I + Ni * Mz * E * 16.0, "flops": Ni * Mz * E * (8 * fx + 15.0 * Mx)},
@@ -160,7 +172,7 @@ def _blas_threads():
 def cpu_baseline(cfg):
     """The oracle as it stands on the host cores: a bounded sample (about 10-30 s) of the bench workload."""
     from oracle.dns_oracle import Oracle
-    Es, nst = min(16, cfg.E), 8
+    Es, nst = (min(16, cfg.E), 8) if cfg.Nx * cfg.Ny * cfg.Nz < 60000 else (min(8, cfg.E), 4)
     o = Oracle(*inputs.plan_args(cfg, E=Es))
     st = inputs.make_state(cfg, range(Es))
     o.set_state(st["vhat"], st["etahat"], st["U00"], st["W00"])
@@ -174,9 +186,13 @@ def cpu_baseline(cfg):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=200)
-    ap.add_argument("--warmup", type=int, default=20)
-    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config number (1-based); 2 = configs[1]")
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--config", type=int, default=4,
+                    help="BASELINE.json config number (1-based); 4 = configs[3], the largest single-GPU workload")
+    ap.add_argument("--form", default="both", choices=["both", "convective", "rotational"],
+                    help="nonlinear term: the headline is the paper's convective form; 'both' adds the rotational "
+                         "form (row f1) as a second measurement in the same line")
     ap.add_argument("--members", type=int, default=0, help="override E per GPU (config 5 sweep)")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -203,23 +219,28 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     base = inputs.CONFIGS[5 if args.sweep else args.config]
     sizes = list(inputs.SWEEP_E) if args.sweep else [args.members or base.E]
-    for E_gpu in sizes:
-        if args.sweep:
-            args.steps, args.warmup = 50, 5                  # BASELINE config 5: 50 steps per ensemble size
-        cfg_all = base.with_E(E_gpu * world)                 # weak scaling: E_gpu members on every rank
-        mine = shard.member_range(cfg_all.E, rank, world)
-        cfg = base.with_E(len(mine))
-        plan = binding.Plan(*inputs.plan_args(cfg), device=f"cuda:{local}")
-        st = inputs.make_state(cfg_all, mine)
+    hbm_peak, peak_src = measured_peaks()
+    fp64 = {"dfma_tflops": None, "dmma_tflops": None}
+    for kind, key in ((0, "dfma_tflops"), (1, "dmma_tflops")):
+        st_, tf = binding.dns_debug_fp64_peak(kind, 0.4)
+        if st_ == binding.DNS_OK:
+            fp64[key] = tf
+    fp64_peak = max([v for v in fp64.values() if v] or [FP64_PEAK_FALLBACK])
+    fp64_src = ("fp64 %.1f TFLOP/s measured live (dns_debug_fp64_peak: DFMA %.1f, DMMA.8x8x4 %.1f; 0.4 s each)"
+                % (fp64_peak, fp64["dfma_tflops"] or 0.0, fp64["dmma_tflops"] or 0.0)) if fp64["dfma_tflops"] \
+        else "fp64 %.1f TFLOP/s fallback (units x clock)" % FP64_PEAK_FALLBACK
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def measure(cfg, cfg_all, st, rot):
+        """Device-resident timing of args.steps steps + per-kernel-class durations, one form of the nonlinear term."""
+        plan = binding.Plan(*inputs.plan_args(cfg), device=f"cuda:{local}",
+                            form=binding.DNS_FORM_ROTATIONAL if rot else binding.DNS_FORM_CONVECTIVE)
         plan.set_state(st["vhat"], st["etahat"], st["U00"], st["W00"])
         stream = torch.cuda.current_stream()
-
-        def barrier():
-            if world > 1:
-                dist.barrier()
-            torch.cuda.synchronize()
-
-        # ---- device-resident timing: W warm-up steps, then exactly K steps between two events
         plan.step(args.warmup)
         barrier()
         sampler = ClockSampler(local)
@@ -233,79 +254,127 @@ def main():
         clocks = sampler.stop()
         ms_max = shard.max_over_ranks(ms) if world > 1 else ms
         value = cfg_all.E * args.steps / (ms_max * 1e-3)
-
-        # ---- per-kernel-class durations with CUDA events on the same stream (live, same state)
+        # per-kernel-class durations with CUDA events on the same stream (live, same state)
         nprof = min(max(args.steps // 10, 3), 20)
         prof = plan.step_profile(nprof)
-        counts = workload_counts(cfg, cfg.E)
-        hbm_peak, peak_src = measured_peaks()
+        counts = workload_counts(cfg, cfg.E, rot)
         kernels = {}
         for name, msum in prof.items():
             per_launch_s = msum * 1e-3 / (3 * nprof)
             c = counts[name]
-            t_hbm, t_alu = c["bytes"] / (hbm_peak * 1e9), c["flops"] / (FP64_PEAK_TFLOPS * 1e12)
+            t_hbm, t_alu = c["bytes"] / (hbm_peak * 1e9), c["flops"] / (fp64_peak * 1e12)
             kernels[name] = {"us_per_launch": per_launch_s * 1e6, "share": msum / max(sum(prof.values()), 1e-30),
                              "GBps": c["bytes"] / per_launch_s * 1e-9, "TFLOPs": c["flops"] / per_launch_s * 1e-12,
+                             "alg_bytes_per_launch": c["bytes"], "alg_flops_per_launch": c["flops"],
                              "bound": "hbm" if t_hbm >= t_alu else "fp64",
                              "frac": max(t_hbm, t_alu) / per_launch_s}
+        return plan, value, ms_max, clocks, kernels
+
+    def roofline_of(kernels, cfg, rot):
         dom = max(kernels, key=lambda k: kernels[k]["share"])
         kd = kernels[dom]
-        traffic = None
+        traffic, tsrc = None, None
         tpath = os.path.join(ROOT, "profiles", "dominant_kernel_traffic.json")
-        if os.path.exists(tpath):
-            try:
-                tj = json.load(open(tpath))
-                if tj.get("kernel") == dom and tj.get("workload") == cfg.name:
-                    traffic = tj.get("dram_bytes_per_launch")
-            except Exception:
-                traffic = None
+        try:
+            for rec in json.load(open(tpath)):
+                if rec.get("kernel") == dom and rec.get("workload") == cfg.name and \
+                        rec.get("form", "convective") == ("rotational" if rot else "convective"):
+                    traffic, tsrc = rec.get("dram_bytes_per_launch"), rec.get("source")
+        except Exception:
+            pass
         if kd["bound"] == "hbm":
-            roofline = {"bound": "hbm", "achieved": kd["GBps"], "peak": hbm_peak, "unit": "GB/s",
-                        "frac": kd["GBps"] / hbm_peak, "traffic": traffic}
+            r = {"bound": "hbm", "achieved": kd["GBps"], "peak": hbm_peak, "unit": "GB/s", "frac": kd["GBps"] / hbm_peak}
         else:
-            roofline = {"bound": "tensor" if dom == "ypair_dmma" else "alu", "achieved": kd["TFLOPs"],
-                        "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": kd["TFLOPs"] / FP64_PEAK_TFLOPS,
-                        "traffic": traffic}
-        roofline.update({"kernel": dom, "peak_source": peak_src + "; fp64 37.0 TFLOP/s measured DMMA/DFMA microbenchmark",
-                         "us_per_launch": kd["us_per_launch"], "share_of_step": kd["share"]})
+            r = {"bound": "tensor" if dom == "ypair_dmma" else "alu", "achieved": kd["TFLOPs"], "peak": fp64_peak,
+                 "unit": "TFLOP/s", "frac": kd["TFLOPs"] / fp64_peak}
+        r.update({"traffic": traffic, "traffic_source": tsrc, "kernel": dom, "peak_source": peak_src + "; " + fp64_src,
+                  "alg_bytes_per_launch": kd["alg_bytes_per_launch"], "us_per_launch": kd["us_per_launch"],
+                  "share_of_step": kd["share"]})
+        return r
 
-        # ---- end to end through the C ABI with HOST (pinned) buffers: H2D + step + D2H every step
-        pin = [torch.from_numpy(np.ascontiguousarray(st[k])).pin_memory() for k in ("vhat", "etahat", "U00", "W00")]
-        outs = [torch.empty_like(t).pin_memory() for t in pin]
-        h2d = sum(t.numel() * t.element_size() for t in pin)
-        d2h = sum(t.numel() * t.element_size() for t in outs)
-        ne2e = min(args.steps, 20)
-        for _ in range(2):
-            plan.set_state(*pin)
-            plan.step(1)
-            plan.get_state(outs)
-        barrier()
-        t0 = time.perf_counter()
-        for _ in range(ne2e):
-            plan.set_state(*pin)
-            plan.step(1)
-            plan.get_state(outs)
-        barrier()
-        e2e_s = time.perf_counter() - t0
+    def measure_e2e(cfg, cfg_all, st, nchunk):
+        """End to end through the C ABI with HOST (pinned) buffers, every step: dns_set_state(host) + dns_step(1) +
+        dns_get_state(host).  Members are independent, so the ensemble is cut into `nchunk` plans on
+        their own streams, each driven by its own host thread: the copies of one chunk overlap the step of another."""
+        import concurrent.futures as cf
+        bounds = [shard.member_range(cfg.E, c, nchunk) for c in range(nchunk)]
+        bounds = [b for b in bounds if len(b)]
+        work = []
+        for b in bounds:
+            sl = slice(b.start, b.stop)
+            strm = torch.cuda.Stream(device=local)
+            with torch.cuda.stream(strm):
+                pl = binding.Plan(*inputs.plan_args(cfg.with_E(len(b))), device=f"cuda:{local}")
+            pin = [torch.from_numpy(np.ascontiguousarray(st[k][sl])).pin_memory() for k in ("vhat", "etahat", "U00", "W00")]
+            outs = [torch.empty_like(t).pin_memory() for t in pin]
+            work.append((pl, pin, outs))
+        h2d = sum(t.numel() * t.element_size() for _, pin, _ in work for t in pin)
+        d2h = sum(t.numel() * t.element_size() for _, _, outs in work for t in outs)
+        ne2e = max(3, min(args.steps, 10))
+
+        def drive(w, n):
+            torch.cuda.set_device(local)
+            pl, pin, outs = w
+            for _ in range(n):
+                pl.set_state(*pin)
+                pl.step(1)
+                pl.get_state(outs)
+
+        with cf.ThreadPoolExecutor(len(work)) as ex:
+            list(ex.map(lambda w: drive(w, 2), work))
+            barrier()
+            t0 = time.perf_counter()
+            list(ex.map(lambda w: drive(w, ne2e), work))
+            barrier()
+            e2e_s = time.perf_counter() - t0
+        for pl, _, _ in work:
+            pl.close()
         e2e_s = shard.max_over_ranks(e2e_s) if world > 1 else e2e_s
-        e2e = {"value": cfg_all.E * ne2e / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-               "steps": ne2e, "note": "dns_set_state(host pinned) + dns_step(1) + dns_get_state(host pinned) per step"}
+        return {"value": cfg_all.E * ne2e / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "steps": ne2e, "chunks": len(work),
+                "note": "dns_set_state(host pinned) + dns_step(1) + dns_get_state(host pinned) per step and member chunk; "
+                        "%d chunks of members on their own plans, streams and host threads" % len(work)}
+
+    for E_gpu in sizes:
+        if args.sweep:
+            args.steps, args.warmup = 50, 5                  # BASELINE config 5: 50 steps per ensemble size
+        cfg_all = base.with_E(E_gpu * world)                 # weak scaling: E_gpu members on every rank
+        mine = shard.member_range(cfg_all.E, rank, world)
+        cfg = base.with_E(len(mine))
+        st = inputs.make_state(cfg_all, mine)
+        forms = {"both": (False, True), "convective": (False,), "rotational": (True,)}[args.form]
+        if args.sweep:
+            forms = forms[:1]
+        res = {}
+        for rot in forms:
+            plan, value, ms_max, clocks, kernels = measure(cfg, cfg_all, st, rot)
+            res[rot] = dict(value=value, ms_max=ms_max, clocks=clocks, kernels=kernels, launches=plan.launches_per_step(),
+                            ws=plan.workspace_bytes, roofline=roofline_of(kernels, cfg, rot))
+            plan.close()
+        head = res[forms[0]]
+        e2e = measure_e2e(cfg, cfg_all, st, 1 if (args.sweep or cfg.E < 8) else 4)
 
         line = {
-            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "metric": METRIC, "value": head["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": head["ms_max"] / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": cfg.name, "members_per_gpu": cfg.E, "members_total": cfg_all.E,
+                       "nonlinear_form": "rotational" if forms[0] else "convective (PAPER.md:147)",
                        "parallelism": f"member-shards x{world} (no collective in dns_step)",
-                       "l2_policy": "working set %.0f MB per GPU > 126 MB L2 (no flush needed)" % (plan.workspace_bytes / 1e6)
-                       if plan.workspace_bytes > 2 * 126e6 else "working set fits L2; not flushed between steps (stated)",
+                       "l2_policy": "working set %.0f MB per GPU > 126 MB L2 (no flush needed)" % (head["ws"] / 1e6)
+                       if head["ws"] > 2 * 126e6 else "working set fits L2; not flushed between steps (stated)",
                        "input_sha256": st["sha256"][:16]},
-            "clocks": clocks, "e2e": e2e, "gpu_launches": args.steps * plan.launches_per_step(),
-            "roofline": roofline, "kernels": kernels,
+            "clocks": head["clocks"], "e2e": e2e, "gpu_launches": args.steps * head["launches"],
+            "roofline": head["roofline"], "kernels": head["kernels"], "fp64_peak": fp64,
         }
+        if len(forms) > 1:
+            r = res[True]
+            line["rotational"] = {"value": r["value"], "unit": UNIT, "ms_per_step": r["ms_max"] / args.steps,
+                                  "clocks": r["clocks"], "roofline": r["roofline"], "kernels": r["kernels"],
+                                  "note": "same workload, steps and timing with dns_plan_set_form(DNS_FORM_ROTATIONAL), "
+                                          "SURVEY.md 8(f) row f1"}
         if rank == 0 and world == 1 and not args.no_cpu_baseline and not args.sweep:
             line["cpu_baseline"] = cpu_baseline(base)
-        plan.close()
         if rank == 0:
             print(json.dumps(line))
     if world > 1:

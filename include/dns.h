@@ -74,6 +74,42 @@ enum {
 int dns_plan_create(dns_plan** out, int Nx, int Ny, int Nz, int E, double Re, double Lx, double Lz, double dt,
                     int flow);
 
+/* dns_plan_set_form -- form of the nonlinear term.  DNS_FORM_CONVECTIVE (default) is the
+ * paper's u . grad u_i.  DNS_FORM_ROTATIONAL forms H = omega x u instead, omega = curl u:
+ * (u . grad)u = omega x u + grad(|u|^2/2) and Eq. 4-5 are what is left of the momentum equation once
+ * gradients are eliminated (:68), so F and G keep their form with H in place of u . grad u; the mean-flow sources of
+ * Eq. 6-7 become the plane means of H_x and H_z.  6 instead of 11 physical fields are transformed per stage.  The two
+ * forms agree to round-off wherever the wall-normal products are resolved and differ at y-truncation level otherwise.
+ * Call before dns_set_state.  Errors: DNS_EINVAL (null, unknown form), DNS_ESTATE (a state is already set). */
+enum { DNS_FORM_CONVECTIVE = 0, DNS_FORM_ROTATIONAL = 1 };
+int dns_plan_set_form(dns_plan* plan, int form);
+
+/* dns_plan_set_coupling -- ensemble-coupled streamwise-mean flow ("Each
+ * ensemble member shares a common streamwise mean flow, which is updated at every time-step by the perturbation
+ * Reynolds stresses averaged over the ensemble members").  With DNS_COUPLING_STREAMWISE_MEAN every stage replaces the
+ * kx = 0 part of the nonlinear vector (all that forces the streamwise-mean flow) and the mean-flow sources of Eq. 6-7
+ * by their average over ALL members, summed in a fixed order; kx != 0 is untouched.  Members whose kx = 0 components
+ * and U00, W00 are equal in dns_set_state keep them equal.  E_total = members of the whole ensemble: plan E on one
+ * GPU; with members sharded over ranks the sum of the ranks' E, and dns_plan_set_exchange must be given.
+ * Call before dns_set_state.  Errors: DNS_EINVAL (null, unknown mode, E_total < E), DNS_ESTATE. */
+enum { DNS_COUPLING_NONE = 0, DNS_COUPLING_STREAMWISE_MEAN = 1 };
+int dns_plan_set_coupling(dns_plan* plan, int mode, long long E_total);
+
+/* dns_plan_set_exchange -- the one exchange step of the path (coupled ensembles sharded over GPUs): fn must replace
+ * dev_buf[0..count) (doubles, DEVICE memory inside the bound workspace) by its element-wise sum over all ranks, ordered
+ * after the work already enqueued on cuda_stream and before anything enqueued later (e.g. an NCCL all-reduce on that
+ * stream), and return 0 on success.  It is called once per stage (3 times per step) from dns_step; count is
+ * (3 Ny (Nz-1) + Ny 3Nz/2) * 2.  With an exchange set dns_step launches directly (a host call cannot be replayed from a
+ * CUDA graph).  fn = NULL removes it.  ctx is passed back verbatim and never dereferenced by the library. */
+typedef int (*dns_exchange_fn)(void* ctx, double* dev_buf, size_t count, void* cuda_stream);
+int dns_plan_set_exchange(dns_plan* plan, dns_exchange_fn fn, void* ctx);
+
+/* dns_add_increment -- state += (dvhat, detahat) between two steps (layout of dns_set_state; host or device): how a
+ * caller applies one realisation of a stochastic forcing (the realisations are the caller's).  The
+ * result is normalised as in dns_set_state (wall rows, (0,0) column, Hermitian kx = 0 plane) and the transform inputs
+ * are re-derived; time, step count and the Poiseuille target flux are kept.  Errors: DNS_EINVAL, DNS_ESTATE, DNS_ECUDA. */
+int dns_add_increment(dns_plan* plan, const double* dvhat, const double* detahat);
+
 /* Bytes of DEVICE workspace the caller must provide to dns_plan_bind (state, stage buffers, transform
  * intermediates).  0 if plan is null. */
 size_t dns_plan_workspace_bytes(const dns_plan* plan);

@@ -13,10 +13,10 @@ extern "C" {
 
 /* dns_debug_fetch -- test hook: copy one INTERNAL device array to a host buffer, synchronising first.  Internal
  * spectral layout is [Ny][nkx][nkz][E] complex128 (member index fastest).  which: 0 u, 1 w, 2 du/dy, 3 dw/dy
- * (current stage, Eq. 17-18), 4 the three spectral advection terms (u.grad)u,(u.grad)v,(u.grad)w back to back,
+ * (current stage, Eq. 17-18; in the rotational form 2 is omega_z = i kx v - du/dy and 3 is omega_x = dw/dy - i kz v), 4 the three spectral advection terms (u.grad)u,(u.grad)v,(u.grad)w back to back,
  * 5 F and 6 G history (Eq. 4-5, interior rows: F^0 after stage 0, F^0 + 4 F^1 after stage 1), 7 v of
  * the current stage, 8 U00 and
- * 9 W00 of the current stage as [Ny][E] float64.  nbytes must equal the array size (DNS_EINVAL otherwise). */
+ * 9 W00 of the current stage as [Ny][E] float64, 10 eta of the current stage (rotational form only; stages 0 and 1).  nbytes must equal the array size (DNS_EINVAL otherwise). */
 int dns_debug_fetch(dns_plan* plan, int which, void* host_dst, size_t nbytes);
 
 /* dns_debug_stage -- test hook: enqueue ONE Crank-Nicolson/RK3 stage (0, 1 or 2) on the

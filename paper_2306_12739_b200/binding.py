@@ -15,17 +15,21 @@ import numpy as np
 
 DNS_COUETTE, DNS_POISEUILLE_CMF = 0, 1
 DNS_OK, DNS_EINVAL, DNS_ENOMEM, DNS_ECUDA, DNS_ENONFINITE, DNS_ESTATE = 0, -1, -2, -3, -4, -5
+DNS_FORM_CONVECTIVE, DNS_FORM_ROTATIONAL = 0, 1
+DNS_COUPLING_NONE, DNS_COUPLING_STREAMWISE_MEAN = 0, 1
 DNS_NCLASS = 4
 CLASS_NAMES = ("fft_z_inv", "line_fft_x_products", "fft_z_fwd", "ypair_dmma")
 
 _LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libdns_b200.so")
 _lib = None
 
-EXPORTS = ("dns_plan_create", "dns_plan_workspace_bytes", "dns_plan_bind", "dns_set_state", "dns_step",
+# every symbol include/dns.h declares, then the test / measurement hooks of include/dns_debug.h
+EXPORTS = ("dns_plan_create", "dns_plan_set_form", "dns_plan_set_coupling", "dns_plan_set_exchange", "dns_add_increment",
+           "dns_plan_workspace_bytes", "dns_plan_bind", "dns_set_state", "dns_step",
            "dns_step_profile", "dns_get_state", "dns_diagnostics", "dns_stats_reset", "dns_stats_accumulate", "dns_stats_get",
-           "dns_debug_fetch", "dns_debug_stage", "dns_launches_per_step",
-           "dns_plan_destroy",
-           "dns_strerror")
+           "dns_launches_per_step", "dns_plan_destroy", "dns_strerror",
+           "dns_debug_fetch", "dns_debug_stage", "dns_debug_set_option", "dns_debug_fp64_peak")
+EXCHANGE_FN = ctypes.CFUNCTYPE(ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p)
 
 
 class DnsError(RuntimeError):
@@ -75,6 +79,18 @@ def lib():
         L.dns_plan_destroy.restype = i
         L.dns_strerror.argtypes = [i]
         L.dns_strerror.restype = ctypes.c_char_p
+        L.dns_plan_set_form.argtypes = [vp, i]
+        L.dns_plan_set_form.restype = i
+        L.dns_plan_set_coupling.argtypes = [vp, i, ctypes.c_longlong]
+        L.dns_plan_set_coupling.restype = i
+        L.dns_plan_set_exchange.argtypes = [vp, EXCHANGE_FN, vp]
+        L.dns_plan_set_exchange.restype = i
+        L.dns_add_increment.argtypes = [vp, dp, dp]
+        L.dns_add_increment.restype = i
+        L.dns_debug_set_option.argtypes = [ctypes.c_char_p, i]
+        L.dns_debug_set_option.restype = i
+        L.dns_debug_fp64_peak.argtypes = [i, d, ctypes.POINTER(d)]
+        L.dns_debug_fp64_peak.restype = i
         _lib = L
     return _lib
 
@@ -98,6 +114,33 @@ def dns_plan_create(Nx, Ny, Nz, E, Re, Lx, Lz, dt, flow):
     st = lib().dns_plan_create(ctypes.byref(h), int(Nx), int(Ny), int(Nz), int(E), float(Re), float(Lx), float(Lz),
                                float(dt), int(flow))
     return st, h
+
+
+def dns_plan_set_form(h, form: int) -> int:
+    return lib().dns_plan_set_form(h, int(form))
+
+
+def dns_plan_set_coupling(h, mode: int, E_total: int) -> int:
+    return lib().dns_plan_set_coupling(h, int(mode), int(E_total))
+
+
+def dns_plan_set_exchange(h, fn) -> int:
+    """fn: an EXCHANGE_FN instance (the caller keeps it alive) or None."""
+    return lib().dns_plan_set_exchange(h, fn if fn is not None else EXCHANGE_FN(0), None)
+
+
+def dns_add_increment(h, dvhat, detahat) -> int:
+    return lib().dns_add_increment(h, _ptr(dvhat), _ptr(detahat))
+
+
+def dns_debug_set_option(name: str, value: int) -> int:
+    return lib().dns_debug_set_option(name.encode(), int(value))
+
+
+def dns_debug_fp64_peak(kind: int, seconds: float):
+    t = ctypes.c_double(0.0)
+    st = lib().dns_debug_fp64_peak(int(kind), float(seconds), ctypes.byref(t))
+    return st, float(t.value)
 
 
 def dns_plan_workspace_bytes(h) -> int:
@@ -161,7 +204,11 @@ def dns_plan_destroy(h) -> int:
 class Plan:
     """dns_plan_create + a torch-allocated workspace bound on torch's current stream."""
 
-    def __init__(self, Nx, Ny, Nz, E, Re, Lx, Lz, dt, flow, device="cuda:0"):
+    def __init__(self, Nx, Ny, Nz, E, Re, Lx, Lz, dt, flow, device="cuda:0", form=DNS_FORM_CONVECTIVE,
+                 coupling=DNS_COUPLING_NONE, E_total=None, allreduce=None):
+        """form / coupling: dns_plan_set_form / dns_plan_set_coupling.  allreduce (coupled ensembles sharded over ranks):
+        a callable taking a float64 torch tensor that views the exchange buffer and summing it over all ranks in place
+        (e.g. shard.allreduce_sum_); E_total = members over all ranks."""
         import torch
 
         self.shape = (int(E), int(Nx) // 2, int(Nz) - 1, int(Ny))
@@ -183,6 +230,23 @@ class Plan:
         if st != DNS_OK:
             raise DnsError(st, "dns_plan_bind")
         self.workspace_bytes = nbytes
+        self._exchange_cb = None
+        if form != DNS_FORM_CONVECTIVE:
+            self._chk(dns_plan_set_form(h, form), "dns_plan_set_form")
+        if coupling != DNS_COUPLING_NONE:
+            self._chk(dns_plan_set_coupling(h, coupling, int(E) if E_total is None else int(E_total)), "dns_plan_set_coupling")
+            if allreduce is not None:
+                ws, base_ptr = self.workspace, self.workspace.data_ptr()
+
+                def _cb(ctx, dev_buf, count, stream):                 # marshalling only: a tensor view of the buffer
+                    try:
+                        off = int(dev_buf) - base_ptr
+                        allreduce(ws[off:off + 8 * int(count)].view(torch.float64))
+                        return 0
+                    except Exception:                                  # nothing may propagate through the C frames
+                        return 1
+                self._exchange_cb = EXCHANGE_FN(_cb)
+                self._chk(dns_plan_set_exchange(h, self._exchange_cb), "dns_plan_set_exchange")
 
     def _chk(self, st, where):
         if st != DNS_OK:
@@ -197,6 +261,13 @@ class Plan:
             assert vhat.shape == self.shape and etahat.shape == self.shape
             assert U00.shape == (self.E, self.Ny) and W00.shape == (self.E, self.Ny)
         self._chk(dns_set_state(self.h, vhat, etahat, U00, W00), "dns_set_state")
+
+    def add_increment(self, dvhat, detahat):
+        if isinstance(dvhat, np.ndarray):
+            dvhat = np.ascontiguousarray(dvhat, dtype=np.complex128)
+            detahat = np.ascontiguousarray(detahat, dtype=np.complex128)
+            assert dvhat.shape == self.shape and detahat.shape == self.shape
+        self._chk(dns_add_increment(self.h, dvhat, detahat), "dns_add_increment")
 
     def step(self, nsteps=1):
         self._chk(dns_step(self.h, nsteps), "dns_step")
@@ -223,6 +294,10 @@ class Plan:
     def debug_fetch(self, which):
         """Internal arrays (test hook): spectral ones come back in ABI order [E][nkx][nkz][Ny]."""
         E, nkx, nkz, Ny = self.shape
+        if which == 10:
+            out = np.empty((1, Ny, nkx, nkz, E), np.complex128)
+            self._chk(dns_debug_fetch(self.h, which, out), "dns_debug_fetch")
+            return np.ascontiguousarray(out.transpose(0, 4, 2, 3, 1))[0]
         if which in (8, 9):
             out = np.empty((Ny, E))
             self._chk(dns_debug_fetch(self.h, which, out), "dns_debug_fetch")

@@ -8,8 +8,9 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libdns_b200.so")
-SOURCES = ["api.cu", "plan.cu", "kernels_fft.cu", "kernels_line.cu", "kernels_y.cu"]
-HEADERS = ["dns_internal.h", "fft_codelets.cuh", "fft_consts.h", os.path.join("..", "..", "include", "dns.h")]
+SOURCES = ["api.cu", "plan.cu", "kernels_fft.cu", "kernels_line.cu", "kernels_y.cu", "peak_fp64.cu"]
+HEADERS = ["dns_internal.h", "fft_codelets.cuh", "fft_consts.h", os.path.join("..", "..", "include", "dns.h"),
+           os.path.join("..", "..", "include", "dns_debug.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "--expt-relaxed-constexpr",
     "-Xcompiler", "-fPIC,-fopenmp,-O2", "-Xptxas", "-v",
@@ -30,11 +31,12 @@ def _stale() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
+def build(force: bool = False, verbose: bool = False, extra_flags=()) -> str:
+    """extra_flags: additional nvcc flags for experiments (e.g. -DDNS_YP_REGCAP=112); the product build passes none."""
     if not force and not _stale():
         return LIB
-    nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    extra_env = os.environ.get("DNS_NVCC_EXTRA", "").split()          # experiments only (e.g. -DDNS_YP_REGCAP=112)
+    nvcc = "/usr/local/cuda/bin/nvcc"
+    extra_env = list(extra_flags)
     objs = []
     procs = []
     os.makedirs(os.path.join(HERE, "build"), exist_ok=True)
@@ -63,4 +65,5 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv,
+                extra_flags=[a for a in sys.argv[1:] if a.startswith("-D") or a.startswith("-X") or a.startswith("--max")]))

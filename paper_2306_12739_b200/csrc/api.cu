@@ -4,11 +4,16 @@
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
+#include <cstring>
 #include <new>
 
 #include "dns_internal.h"
 
 namespace {
+
+// test / tuning options of include/dns_debug.h (process-wide; -1 = default)
+struct Option { const char* name; int value; };
+Option g_options[] = {{"graph", -1}, {"zreg", -1}, {"etf", -1}, {"ety", -1}, {"nty", -1}, {"line_tps", -1}};
 
 size_t align256(size_t b) { return (b + 255) & ~(size_t)255; }
 
@@ -36,7 +41,7 @@ size_t carve_workspace(dns_plan* p, void* base) {
     DnsDev& d = p->d;
     Carve c{static_cast<char*>(base)};
     const size_t S = d.S, I = d.Isz, NE = (size_t)d.Ny * d.E;
-    d.vt = c.take<double2>(S);  d.et = c.take<double2>(S);  d.vs = c.take<double2>(S);
+    d.vt = c.take<double2>(S);  d.et = c.take<double2>(S);  d.vs = c.take<double2>(S);  d.es = c.take<double2>(S);
     d.uh = c.take<double2>(S);  d.wh = c.take<double2>(S);  d.duh = c.take<double2>(S);  d.dwh = c.take<double2>(S);
     d.Nh = c.take<double2>(3 * S);
     d.F0 = c.take<double2>(S);  d.G0 = c.take<double2>(S);
@@ -44,6 +49,7 @@ size_t carve_workspace(dns_plan* p, void* base) {
     d.I3 = c.take<double2>(3 * I);
     d.uvpart = c.take<double2>((size_t)d.Ny * d.Mz * d.E);
     d.uvc0 = c.take<double2>(NE);
+    d.ens = c.take<double2>(dns_ens_count(d) / 2);
     d.Ut = c.take<double>(NE);  d.Wt = c.take<double>(NE);  d.Us = c.take<double>(NE);  d.Ws = c.take<double>(NE);
     d.gamma = c.take<double>(d.E);  d.Qstar = c.take<double>(d.E);
     d.diag = c.take<double>((size_t)d.E * 6 + NE);
@@ -64,32 +70,51 @@ bool is_device_ptr(const void* q) {
     return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
 }
 
-void run_stage(dns_plan* p, int s, cudaEvent_t* ev) {
-    // ev (optional): 5 events bracketing the 4 kernel launches (the mean flow rides inside the per-pair launch)
+int run_stage(dns_plan* p, int s, cudaEvent_t* ev) {
+    // ev (optional): 5 events bracketing the 4 kernel classes (the mean flow rides beside the per-pair launch)
     const double2* vin = s == 0 ? p->d.vt : p->d.vs;
+    const double2* ein = s == 0 ? p->d.et : p->d.es;
+    const bool coupled = p->d.coupling == DNS_COUPLING_STREAMWISE_MEAN;
     if (ev) cudaEventRecord(ev[0], p->stream);
-    launch_zinv(p, vin);
+    launch_zinv(p, vin, ein);
     if (ev) cudaEventRecord(ev[1], p->stream);
     launch_line(p);
-    // the mean flow (row a10) needs only the plane sums of the line kernel: fork it onto the side stream, join at the end
-    cudaEventRecord(p->ev_fork, p->stream);
-    cudaStreamWaitEvent(p->side, p->ev_fork, 0);
-    launch_mean(p, s, 0, p->side);
-    cudaEventRecord(p->ev_join, p->side);
     if (ev) cudaEventRecord(ev[2], p->stream);
+    // the mean flow (row a10) needs only the plane sums of the line kernel: fork it onto the side stream, join at the end.
+    // Coupled ensemble (row f2): it must wait for the ensemble means, which follow the z-forward transform.
+    if (!coupled) {
+        cudaEventRecord(p->ev_fork, p->stream);
+        cudaStreamWaitEvent(p->side, p->ev_fork, 0);
+        launch_mean(p, s, 0, p->side);
+        cudaEventRecord(p->ev_join, p->side);
+    }
     launch_zfwd(p);
     if (ev) cudaEventRecord(ev[3], p->stream);
+    if (coupled) {
+        if (p->exchange) {
+            launch_ens(p, 0);
+            if (p->exchange(p->exchange_ctx, reinterpret_cast<double*>(p->d.ens), dns_ens_count(p->d), p->stream) != 0) return DNS_ECUDA;
+            launch_ens(p, 1);
+        } else {
+            launch_ens(p, 2);
+        }
+        cudaEventRecord(p->ev_fork, p->stream);
+        cudaStreamWaitEvent(p->side, p->ev_fork, 0);
+        launch_mean(p, s, 0, p->side);
+        cudaEventRecord(p->ev_join, p->side);
+    }
     launch_ypair(p, s, 0);
     cudaStreamWaitEvent(p->stream, p->ev_join, 0);
     if (ev) cudaEventRecord(ev[4], p->stream);
+    return DNS_OK;
 }
 
 // Captures one time step into a CUDA graph (on an internal stream: the plan's stream may be the legacy default stream,
 // which cannot be captured).  On any failure the plan falls back to direct launches for good.
 void build_step_graph(dns_plan* p) {
     p->graph_state = -1;
-    if (getenv("DNS_GRAPH") && atoi(getenv("DNS_GRAPH")) == 0) return;
-    if (cudaGetLastError() != cudaSuccess) return;
+    if (dns_option("graph") == 0 || p->exchange) return;
+    if (cudaPeekAtLastError() != cudaSuccess) return;     // a pending error is reported by the caller, not cleared here
     if (!p->capture_stream && cudaStreamCreateWithFlags(&p->capture_stream, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); return; }
     cudaStream_t user = p->stream;
     if (cudaStreamBeginCapture(p->capture_stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { cudaGetLastError(); return; }
@@ -151,6 +176,7 @@ int dns_plan_create(dns_plan** out, int Nx, int Ny, int Nz, int E, double Re, do
     d.Nx = Nx; d.Ny = Ny; d.Nz = Nz; d.E = E; d.Mx = Mx; d.Mz = Mz;
     d.nkx = Nx / 2; d.nkz = Nz - 1; d.nzh = Nz / 2; d.P = d.nkx * d.nkz; d.Ni = Ny - 2; d.flow = flow;
     d.dt = dt; d.Re = Re; d.Uw = flow == DNS_COUETTE ? 1.0 : 0.0; d.invMxMz = 1.0 / ((double)Mx * Mz);
+    d.form = DNS_FORM_CONVECTIVE; d.coupling = DNS_COUPLING_NONE; d.invEtot = 1.0 / E;
     d.S = (size_t)Ny * d.P * E;
     {
         const int tps = dns_line_tps(Mx, E);             // lanes per slot of the line kernel = largest member tile
@@ -164,16 +190,16 @@ int dns_plan_create(dns_plan** out, int Nx, int Ny, int Nz, int E, double Re, do
     p->Lx = Lx; p->Lz = Lz;
     // member tiles
     p->ETf = pow2ceil(E) < 32 ? pow2ceil(E) : 32;
-    if (const char* s = getenv("DNS_ETF")) { int v = atoi(s); if ((v == 4 || v == 8 || v == 16 || v == 32) && v <= pow2ceil(E)) p->ETf = v; }
+    { const int v = dns_option("etf"); if ((v == 4 || v == 8 || v == 16 || v == 32) && v <= pow2ceil(E)) p->ETf = v; }
     d.Kp = (((d.Ni + 1) / 2 + 7) / 8) * 8;
     int ETy = pow2ceil(E) < 16 ? pow2ceil(E) : 16;
     if (ETy < 4) ETy = 4;
     while (ETy > 4 && dns_ypair_smem(d.Ni, Ny, ETy) > 75 * 1024) ETy >>= 1;
-    if (const char* s = getenv("DNS_ETY")) { int v = atoi(s); if (v == 4 || v == 8 || v == 16) ETy = v; }
+    { const int v = dns_option("ety"); if (v == 4 || v == 8 || v == 16) ETy = v; }
     if (dns_ypair_smem(d.Ni, Ny, ETy) > 227 * 1024) { delete p; return DNS_EINVAL; }
     p->ETy = ETy;
     p->NTy = ETy >= 8 ? 2 : 1;
-    if (const char* s = getenv("DNS_NTY")) { int v = atoi(s); if ((v == 1 || v == 2 || v == 4) && 4 * v <= ETy) p->NTy = v; }
+    { const int v = dns_option("nty"); if ((v == 1 || v == 2 || v == 4) && 4 * v <= ETy) p->NTy = v; }
     while (32 * (d.Kp / 8) * (ETy / (4 * p->NTy)) > 1024) p->NTy *= 2;
     if (cudaStreamCreateWithFlags(&p->side, cudaStreamNonBlocking) != cudaSuccess ||
         cudaEventCreateWithFlags(&p->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
@@ -213,6 +239,30 @@ int dns_plan_bind(dns_plan* p, void* ws, size_t bytes, void* stream) {
     return cuda_status(p, cudaMemsetAsync(ws, 0, p->workspace_bytes, p->stream));
 }
 
+// copies up to four ABI arrays into the staging area; *all_dev = every given pointer is a device pointer
+static cudaError_t stage_in(dns_plan* p, const double* vhat, const double* etahat, const double* U00, const double* W00,
+                            bool* all_dev) {
+    DnsDev& d = p->d;
+    const size_t S = d.S, NE = (size_t)d.Ny * d.E;
+    double2* sv = d.stage_io;
+    double2* se = sv + S;
+    double* sU = reinterpret_cast<double*>(se + S);
+    double* sW = sU + NE;
+    cudaError_t e = cudaSuccess;
+    *all_dev = true;
+    auto in = [&](void* dst, const void* src, size_t bytes) {
+        if (!src || e != cudaSuccess) return;
+        const bool dev = is_device_ptr(src);
+        if (!dev) *all_dev = false;
+        e = cudaMemcpyAsync(dst, src, bytes, dev ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, p->stream);
+    };
+    in(sv, vhat, S * sizeof(double2));
+    in(se, etahat, S * sizeof(double2));
+    in(sU, U00, NE * sizeof(double));
+    in(sW, W00, NE * sizeof(double));
+    return e;
+}
+
 int dns_set_state(dns_plan* p, const double* vhat, const double* etahat, const double* U00, const double* W00) {
     if (!p || !vhat || !etahat || !U00 || !W00) return DNS_EINVAL;
     if (p->sticky != DNS_OK) return p->sticky;
@@ -223,24 +273,67 @@ int dns_set_state(dns_plan* p, const double* vhat, const double* etahat, const d
     double2* se = sv + S;
     double* sU = reinterpret_cast<double*>(se + S);
     double* sW = sU + NE;
-    const bool dev = is_device_ptr(vhat);
-    const cudaMemcpyKind kind = dev ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
-    cudaError_t e = cudaMemcpyAsync(sv, vhat, S * sizeof(double2), kind, p->stream);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(se, etahat, S * sizeof(double2), is_device_ptr(etahat) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, p->stream);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(sU, U00, NE * sizeof(double), is_device_ptr(U00) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, p->stream);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(sW, W00, NE * sizeof(double), is_device_ptr(W00) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, p->stream);
+    bool all_dev = true;
+    cudaError_t e = stage_in(p, vhat, etahat, U00, W00, &all_dev);
     if (e != cudaSuccess) return cuda_status(p, e);
-    launch_abi_to_internal(p, sv, d.vt);
-    launch_abi_to_internal(p, se, d.et);
+    launch_abi_to_internal(p, sv, d.vt, 0);
+    launch_abi_to_internal(p, se, d.et, 0);
     launch_normalise_state(p);
     launch_mean_in(p, sU, sW);
-    launch_ypair(p, 0, 1);          // derive u, w, du/dy, dw/dy of the initial state (Eq. 17-18)
+    launch_ypair(p, 0, 1);          // derive u, w, du/dy, dw/dy (or omega_x, omega_z) of the initial state (Eq. 17-18)
     launch_mean(p, 0, 1, p->stream);   // and their (0,0) column
     p->has_state = true;
     p->nsteps_done = 0;
     e = cudaGetLastError();
-    if (e == cudaSuccess && !dev) e = cudaStreamSynchronize(p->stream);
+    // any host source: its copy may still be in flight (pinned memory), so the call only returns once it has landed
+    if (e == cudaSuccess && !all_dev) e = cudaStreamSynchronize(p->stream);
     return cuda_status(p, e);
+}
+
+int dns_add_increment(dns_plan* p, const double* dv, const double* deta) {
+    if (!p || !dv || !deta) return DNS_EINVAL;
+    if (p->sticky != DNS_OK) return p->sticky;
+    if (!p->bound || !p->has_state) return DNS_ESTATE;
+    DnsDev& d = p->d;
+    double2* sv = d.stage_io;
+    double2* se = sv + d.S;
+    bool all_dev = true;
+    cudaError_t e = stage_in(p, dv, deta, nullptr, nullptr, &all_dev);
+    if (e != cudaSuccess) return cuda_status(p, e);
+    launch_abi_to_internal(p, sv, d.vt, 1);            // accumulate
+    launch_abi_to_internal(p, se, d.et, 1);
+    launch_normalise_state(p);
+    launch_ypair(p, 0, 1);
+    launch_mean(p, 0, 1, p->stream);
+    e = cudaGetLastError();
+    if (e == cudaSuccess && !all_dev) e = cudaStreamSynchronize(p->stream);
+    return cuda_status(p, e);
+}
+
+int dns_plan_set_form(dns_plan* p, int form) {
+    if (!p || (form != DNS_FORM_CONVECTIVE && form != DNS_FORM_ROTATIONAL)) return DNS_EINVAL;
+    if (p->has_state) return DNS_ESTATE;
+    if (form != p->d.form) drop_step_graph(p);
+    p->d.form = form;
+    return DNS_OK;
+}
+
+int dns_plan_set_coupling(dns_plan* p, int mode, long long E_total) {
+    if (!p || (mode != DNS_COUPLING_NONE && mode != DNS_COUPLING_STREAMWISE_MEAN)) return DNS_EINVAL;
+    if (mode == DNS_COUPLING_STREAMWISE_MEAN && E_total < p->d.E) return DNS_EINVAL;
+    if (p->has_state) return DNS_ESTATE;
+    drop_step_graph(p);
+    p->d.coupling = mode;
+    p->d.invEtot = 1.0 / (double)(mode == DNS_COUPLING_NONE ? p->d.E : E_total);
+    return DNS_OK;
+}
+
+int dns_plan_set_exchange(dns_plan* p, dns_exchange_fn fn, void* ctx) {
+    if (!p) return DNS_EINVAL;
+    drop_step_graph(p);
+    p->exchange = fn;
+    p->exchange_ctx = ctx;
+    return DNS_OK;
 }
 
 int dns_step(dns_plan* p, int nsteps) {
@@ -252,7 +345,8 @@ int dns_step(dns_plan* p, int nsteps) {
         if (p->graph_state == 1) {
             if (cudaGraphLaunch(p->graph_exec, p->stream) != cudaSuccess) return cuda_status(p, cudaGetLastError());
         } else {
-            for (int s = 0; s < 3; ++s) run_stage(p, s, nullptr);
+            for (int s = 0; s < 3; ++s)
+                if (run_stage(p, s, nullptr) != DNS_OK) { p->sticky = DNS_ECUDA; return DNS_ECUDA; }
         }
         ++p->nsteps_done;
     }
@@ -269,7 +363,8 @@ int dns_step_profile(dns_plan* p, int nsteps, double* ms) {
         p->ev_init = true;
     }
     for (int it = 0; it < nsteps; ++it) {
-        for (int s = 0; s < 3; ++s) run_stage(p, s, p->ev + 5 * s);
+        for (int s = 0; s < 3; ++s)
+            if (run_stage(p, s, p->ev + 5 * s) != DNS_OK) { p->sticky = DNS_ECUDA; return DNS_ECUDA; }
         cudaError_t e = cudaStreamSynchronize(p->stream);
         if (e != cudaSuccess) return cuda_status(p, e);
         for (int s = 0; s < 3; ++s)
@@ -383,6 +478,7 @@ int dns_debug_fetch(dns_plan* p, int which, void* dst, size_t nbytes) {
         case 7: src = d.vs; break;
         case 8: src = d.Us; sz = NE; break;
         case 9: src = d.Ws; sz = NE; break;
+        case 10: src = d.es; break;
         default: return DNS_EINVAL;
     }
     if (nbytes != sz) return DNS_EINVAL;
@@ -395,12 +491,23 @@ int dns_debug_stage(dns_plan* p, int stage) {
     if (!p || stage < 0 || stage > 2) return DNS_EINVAL;
     if (p->sticky != DNS_OK) return p->sticky;
     if (!p->bound || !p->has_state) return DNS_ESTATE;
-    run_stage(p, stage, nullptr);
+    if (run_stage(p, stage, nullptr) != DNS_OK) { p->sticky = DNS_ECUDA; return DNS_ECUDA; }
     if (stage == 2) ++p->nsteps_done;
     return cuda_status(p, cudaGetLastError());
 }
 
-int dns_launches_per_step(const dns_plan* p) { return p ? 3 * 5 : 0; }
+int dns_launches_per_step(const dns_plan* p) {
+    if (!p) return 0;
+    const int ens = p->d.coupling == DNS_COUPLING_STREAMWISE_MEAN ? (p->exchange ? 2 : 1) : 0;
+    return 3 * (5 + ens);
+}
+
+int dns_debug_set_option(const char* name, int value) {
+    if (!name) return DNS_EINVAL;
+    for (auto& o : g_options)
+        if (strcmp(o.name, name) == 0) { o.value = value < 0 ? -1 : value; return DNS_OK; }
+    return DNS_EINVAL;
+}
 
 int dns_plan_destroy(dns_plan* p) {
     if (!p) return DNS_OK;
@@ -417,3 +524,9 @@ int dns_plan_destroy(dns_plan* p) {
 }
 
 }  // extern "C"
+
+int dns_option(const char* name) {
+    for (auto& o : g_options)
+        if (strcmp(o.name, name) == 0) return o.value;
+    return -1;
+}

@@ -5,6 +5,7 @@
 #include <vector>
 
 #include "../../include/dns.h"
+#include "../../include/dns_debug.h"
 
 // Everything a kernel needs, passed by value.  Spectral arrays are [Ny][nkx][nkz][E] complex (member index
 // fastest: the paper's vectorised-ensemble axis, is the coalescing axis); mixed (kx, z) arrays
@@ -12,6 +13,9 @@
 // one TMA bulk copy in the line kernel); mean-flow arrays are [Ny][E] real.
 struct DnsDev {
     int Nx, Ny, Nz, E, Mx, Mz, nkx, nkz, nzh, P, Ni, flow;
+    int form;              // DNS_FORM_CONVECTIVE (u . grad u_i) or DNS_FORM_ROTATIONAL (omega x u, row f1)
+    int coupling;          // DNS_COUPLING_NONE or DNS_COUPLING_STREAMWISE_MEAN (row f2)
+    double invEtot;        // 1 / (members of the whole ensemble, over all ranks) for the coupled mean
     int etl, ntl;          // mixed arrays are tile-major: member tile of 2^etl lanes, ntl = ceil(E / 2^etl) tiles
     double dt, Re, Uw, invMxMz;
     // plan-owned constant tables
@@ -32,12 +36,17 @@ struct DnsDev {
     // workspace
     double2 *vt, *et;      // state at time t
     double2* vs;           // v of the current stage (transform input)
-    double2 *uh, *wh, *duh, *dwh;   // u, w, du/dy, dw/dy of the current stage
+    double2* es;           // eta of the current stage (rotational form only: omega_y is a transform input)
+    double2 *uh, *wh;      // u, w of the current stage
+    double2 *duh, *dwh;    // convective: du/dy, dw/dy ; rotational: omega_z = i kx v - du/dy, omega_x = dw/dy - i kz v
     double2* Nh;           // 3 fields: (u.grad)u, (u.grad)v, (u.grad)w in spectral space
     double2 *F0, *G0;      // history of the nonlinear terms: N0 after stage 0, N0 + 4 N1 after stage 1
-    double2* I8;           // 8 mixed-space fields: u v w Du Dw uz vz wz
+    double2* I8;           // mixed-space inputs of the line kernel: u v w Du Dw uz vz wz (convective, 8 fields)
+                           // or u v w omega_x omega_y omega_z (rotational, 6 fields)
     double2* I3;           // 3 mixed-space fields: Nu Nv Nw
-    double2* uvpart;       // [Ny][Mz][E] (sum_x u v, sum_x w v) per z line
+    double2* uvpart;       // [Ny][Mz][E] (sum_x u v, sum_x w v) per z line; rotational: (sum_x H_x, sum_x H_z)
+    double2* ens;          // coupled ensemble (row f2): [3][Ny][nkz] sums over the members of the kx = 0 plane of the
+                           // nonlinear vector, then [Ny][Mz] sums of uvpart -- one contiguous exchange buffer
     double2* uvc0;         // [Ny][E] history of the plane means (as F0, G0)
     double *Ut, *Wt, *Us, *Ws;      // mean profiles at t and at the current stage
     double *gamma, *Qstar; // [E]
@@ -59,7 +68,7 @@ struct dns_plan {
     int R1x = 0, R2x = 0, R1z = 0, R2z = 0;   // four-step factorisations of Mx, Mz
     int ETy = 0, NTy = 0;                      // member tile of the per-pair kernel, n-tiles per warp
     int ETf = 0;                               // member tile of the transform kernels
-    int line_grid = 0;                         // persistent grid of the line kernel (set at first launch)
+    int line_grid = 0, line_grid_form = 0;     // persistent grid of the line kernel (set at first launch, per form)
     int line_tps = 0;                          // lanes per slot of the line kernel (4, 8 or 16)
     alignas(64) unsigned char tmaps[3][128];   // CUtensorMap of Nh, vt, et (encoded at dns_plan_bind)
     cudaStream_t side = nullptr;               // the mean-flow kernel runs here, under the z-forward and per-pair kernels
@@ -69,6 +78,9 @@ struct dns_plan {
     size_t workspace_bytes = 0;
     cudaStream_t stream = nullptr;
     bool bound = false, has_state = false;
+    // coupled ensemble across ranks: sums dev_buf[0..count) over all ranks in place, ordered on the stream (include/dns.h)
+    dns_exchange_fn exchange = nullptr;
+    void* exchange_ctx = nullptr;
     // one time step (15 launches, fork/join with the side stream) captured once into a CUDA graph and replayed:
     // small ensembles are launch-bound.  graph_state: 0 not tried, 1 ready, -1 unavailable (direct launches)
     cudaStream_t capture_stream = nullptr;
@@ -88,14 +100,17 @@ bool dns_factor_len(int M, int* R1, int* R2);
 int dns_line_tps(int Mx, int E);
 
 // kernel launchers (kernels_*.cu); stage = 0,1,2
-void launch_zinv(dns_plan* p, const double2* vin);
+void launch_zinv(dns_plan* p, const double2* vin, const double2* ein);
+void launch_ens(dns_plan* p, int phase);     // phase 0: sums -> d.ens ; 1: d.ens / Etot -> members ; 2: both
+size_t dns_ens_count(const DnsDev& d);       // doubles in d.ens
+int dns_option(const char* name);            // test / tuning options (include/dns_debug.h); -1 = default
 void launch_line(dns_plan* p);
 void launch_zfwd(dns_plan* p);
 void launch_ypair(dns_plan* p, int stage, int derive_only);
 size_t dns_ypair_smem(int Ni, int Ny, int ET);
 int dns_ypair_encode_maps(dns_plan* p);
 void launch_mean(dns_plan* p, int stage, int derive_only, cudaStream_t stream);
-void launch_abi_to_internal(dns_plan* p, const double2* src_abi, double2* dst);
+void launch_abi_to_internal(dns_plan* p, const double2* src_abi, double2* dst, int accumulate);
 void launch_internal_to_abi(dns_plan* p, const double2* src, double2* dst_abi);
 void launch_mean_in(dns_plan* p, const double* U_abi, const double* W_abi);
 void launch_mean_out(dns_plan* p, double* U_abi, double* W_abi);

@@ -26,13 +26,21 @@ __device__ __forceinline__ int pos_to_mi(int pos, int M, int nzh, int nkz) {
     return -1;
 }
 
+// Input field f of the z-inverse transform.  Convective form: u, v, w, du/dy, dw/dy -- u, v, w also give
+// their z-derivative (i kz on load), 8 mixed fields.  Rotational form (row f1): u, v, w, omega_x, omega_y = eta, omega_z,
+// 6 mixed fields in that order, no derivative.
+__device__ __forceinline__ const double2* zinv_src(const DnsDev& d, int f, const double2* vin, const double2* ein) {
+    if (d.form == DNS_FORM_ROTATIONAL) return f == 0 ? d.uh : f == 1 ? vin : f == 2 ? d.wh : f == 3 ? d.dwh : f == 4 ? ein : d.duh;
+    return f == 0 ? d.uh : f == 1 ? vin : f == 2 ? d.wh : f == 3 ? d.duh : d.dwh;
+}
+
 // ------------------------------------------------------------------------------------------------ z inverse
-// grid.x = Ni * nblk_n * ntile_e, grid.y = 5 input fields (u, v, w, Du, Dw); block = 256
+// grid.x = Ni * nblk_n * ntile_e, grid.y = input fields (5 convective, 6 rotational); block = 256
 #ifndef DNS_FFT_MINB
 #define DNS_FFT_MINB 2
 #endif
 template <int R1, int R2>
-__global__ void __launch_bounds__(256, DNS_FFT_MINB) k_zinv(DnsDev d, const double2* __restrict__ vin, int etlog, int NB) {
+__global__ void __launch_bounds__(256, DNS_FFT_MINB) k_zinv(DnsDev d, const double2* __restrict__ vin, const double2* __restrict__ ein, int etlog, int NB) {
     constexpr int M = R1 * R2;
     extern __shared__ double2 sm[];
     const int ET = 1 << etlog, e_l = threadIdx.x & (ET - 1), slot = threadIdx.x >> etlog, nslots = blockDim.x >> etlog;
@@ -44,8 +52,9 @@ __global__ void __launch_bounds__(256, DNS_FFT_MINB) k_zinv(DnsDev d, const doub
     const int f = blockIdx.y;
     const int e = te * ET + e_l, n0 = bn * NB;
     const bool eok = e < d.E;
-    const double2* src = f == 0 ? d.uh : f == 1 ? vin : f == 2 ? d.wh : f == 3 ? d.duh : d.dwh;
-    const int nv = f < 3 ? 2 : 1;                      // u, v, w also produce their z-derivative
+    const bool rot = d.form == DNS_FORM_ROTATIONAL;
+    const double2* src = zinv_src(d, f, vin, ein);
+    const int nv = (!rot && f < 3) ? 2 : 1;            // convective: u, v, w also produce their z-derivative
     double2* tws = sm;                                 // [M] twiddles
     double2* buf = sm + M;                             // [NB*nv][M][ET]
     for (int i = threadIdx.x; i < M; i += blockDim.x) tws[i] = d.twz[i];
@@ -154,7 +163,7 @@ __global__ void __launch_bounds__(256) k_zfwd(DnsDev d, int etlog, int NB) {
 //                                  x(k + H h) = E(k) +- w^k O(k), w = exp(-2 pi i / M) on swapped data (swap identity)
 //   forward (decimation in frequency): thread h holds x(i + H h); a_h(i) = (x(i) +- x(i+H)) w^(h i); X(2m + h) = DFT_H(a_h)(m)
 template <int H, bool TP>
-__global__ void __launch_bounds__(128) k_zinv_r(DnsDev d, const double2* __restrict__ vin) {
+__global__ void __launch_bounds__(128) k_zinv_r(DnsDev d, const double2* __restrict__ vin, const double2* __restrict__ ein) {
     constexpr int M = 2 * H, LO = H / 3, HI = 2 * H / 3;   // positions 2i+h < M/3 <=> i < LO ; > 2M/3 <=> i > HI (i == HI: h = 1 only)
     static_assert(H % 3 == 0, "padded length must be 3/2 of an even grid");
     const int h = threadIdx.x & 1;
@@ -165,13 +174,14 @@ __global__ void __launch_bounds__(128) k_zinv_r(DnsDev d, const double2* __restr
     const int n = ok ? q / d.E : 0, e = ok ? q - n * d.E : 0;
     // TP (two passes): blockIdx.y = input field; u, v, w also give their z-derivative in a second pass over the same
     // inputs (now L1/L2 hits): 3 S less DRAM traffic, more registers.  Otherwise blockIdx.y = one of the 8 outputs.
-    const int f = TP ? blockIdx.y : (blockIdx.y < 5 ? blockIdx.y : blockIdx.y - 5);
-    const double2* src = (f == 0 ? d.uh : f == 1 ? vin : f == 2 ? d.wh : f == 3 ? d.duh : d.dwh) +
-                         ((size_t)j * d.nkx + n) * d.nkz * d.E + e;
+    // Rotational form: blockIdx.y = one of the 6 fields, no derivative pass.
+    const bool rot = d.form == DNS_FORM_ROTATIONAL;
+    const int f = (TP || rot) ? blockIdx.y : (blockIdx.y < 5 ? blockIdx.y : blockIdx.y - 5);
+    const double2* src = zinv_src(d, f, vin, ein) + ((size_t)j * d.nkx + n) * d.nkz * d.E + e;
 #pragma unroll 1
-    for (int pass = 0; pass < (TP && f < 3 ? 2 : 1); ++pass) {
-    const bool deriv = TP ? pass == 1 : blockIdx.y >= 5;
-    const int var = TP ? (deriv ? f + 5 : f) : blockIdx.y;
+    for (int pass = 0; pass < (TP && !rot && f < 3 ? 2 : 1); ++pass) {
+    const bool deriv = rot ? false : (TP ? pass == 1 : blockIdx.y >= 5);
+    const int var = rot ? f : (TP ? (deriv ? f + 5 : f) : blockIdx.y);
     // all loads first (independent, in flight together), then the i kz factor and the swap of the inverse transform
     double2 a[H];
     double kzv[H];
@@ -264,7 +274,7 @@ __device__ __forceinline__ double2 quad_dft4(double2 z, int l1, int l0) {
 }
 
 template <int H, bool TP>
-__global__ void __launch_bounds__(128) k_zinv_r4(DnsDev d, const double2* __restrict__ vin) {
+__global__ void __launch_bounds__(128) k_zinv_r4(DnsDev d, const double2* __restrict__ vin, const double2* __restrict__ ein) {
     constexpr int M = 4 * H, LO = H / 3, HI = 2 * H / 3;   // positions 4i+r < M/3 <=> i < LO ; > 2M/3 <=> i > HI (i == HI: r >= 1)
     static_assert(H % 3 == 0, "padded length must be 3/2 of an even grid");
     const int l0 = threadIdx.x & 1, l1 = (threadIdx.x >> 1) & 1, r = 2 * l1 + l0, qo = l1 + 2 * l0;
@@ -275,13 +285,14 @@ __global__ void __launch_bounds__(128) k_zinv_r4(DnsDev d, const double2* __rest
     const int n = ok ? q / d.E : 0, e = ok ? q - n * d.E : 0;
     // TP (two passes): blockIdx.y = input field; u, v, w also give their z-derivative in a second pass over the same
     // inputs (now L1/L2 hits): 3 S less DRAM traffic, more registers.  Otherwise blockIdx.y = one of the 8 outputs.
-    const int f = TP ? blockIdx.y : (blockIdx.y < 5 ? blockIdx.y : blockIdx.y - 5);
-    const double2* src = (f == 0 ? d.uh : f == 1 ? vin : f == 2 ? d.wh : f == 3 ? d.duh : d.dwh) +
-                         ((size_t)j * d.nkx + n) * d.nkz * d.E + e;
+    // Rotational form: blockIdx.y = one of the 6 fields, no derivative pass.
+    const bool rot = d.form == DNS_FORM_ROTATIONAL;
+    const int f = (TP || rot) ? blockIdx.y : (blockIdx.y < 5 ? blockIdx.y : blockIdx.y - 5);
+    const double2* src = zinv_src(d, f, vin, ein) + ((size_t)j * d.nkx + n) * d.nkz * d.E + e;
 #pragma unroll 1
-    for (int pass = 0; pass < (TP && f < 3 ? 2 : 1); ++pass) {
-    const bool deriv = TP ? pass == 1 : blockIdx.y >= 5;
-    const int var = TP ? (deriv ? f + 5 : f) : blockIdx.y;
+    for (int pass = 0; pass < (TP && !rot && f < 3 ? 2 : 1); ++pass) {
+    const bool deriv = rot ? false : (TP ? pass == 1 : blockIdx.y >= 5);
+    const int var = rot ? f : (TP ? (deriv ? f + 5 : f) : blockIdx.y);
     double2 a[H];
     double kzv[H];
 #pragma unroll
@@ -344,10 +355,10 @@ __global__ void __launch_bounds__(128) k_zfwd_r4(DnsDev d) {
     }
 }
 
-template <int H> void zinv_r4_launch(dns_plan* p, const double2* vin) {
+template <int H> void zinv_r4_launch(dns_plan* p, const double2* vin, const double2* ein) {
     const DnsDev& d = p->d;
-    dim3 grid((unsigned)(d.Ni * ((d.nkx * d.E + 31) / 32)), 8);
-    k_zinv_r4<H, false><<<grid, 128, 0, p->stream>>>(d, vin);
+    dim3 grid((unsigned)(d.Ni * ((d.nkx * d.E + 31) / 32)), d.form == DNS_FORM_ROTATIONAL ? 6 : 8);
+    k_zinv_r4<H, false><<<grid, 128, 0, p->stream>>>(d, vin, ein);
 }
 template <int H> void zfwd_r4_launch(dns_plan* p) {
     const DnsDev& d = p->d;
@@ -355,11 +366,11 @@ template <int H> void zfwd_r4_launch(dns_plan* p) {
     k_zfwd_r4<H><<<grid, 128, 0, p->stream>>>(d);
 }
 
-template <int H> void zinv_r_launch(dns_plan* p, const double2* vin) {
+template <int H> void zinv_r_launch(dns_plan* p, const double2* vin, const double2* ein) {
     const DnsDev& d = p->d;
     constexpr bool TP = H <= 24;                      // measured: helps Mz <= 48, costs occupancy above
-    dim3 grid((unsigned)(d.Ni * ((d.nkx * d.E + 63) / 64)), TP ? 5 : 8);
-    k_zinv_r<H, TP><<<grid, 128, 0, p->stream>>>(d, vin);
+    dim3 grid((unsigned)(d.Ni * ((d.nkx * d.E + 63) / 64)), d.form == DNS_FORM_ROTATIONAL ? 6 : (TP ? 5 : 8));
+    k_zinv_r<H, TP><<<grid, 128, 0, p->stream>>>(d, vin, ein);
 }
 template <int H> void zfwd_r_launch(dns_plan* p) {
     const DnsDev& d = p->d;
@@ -367,11 +378,18 @@ template <int H> void zfwd_r_launch(dns_plan* p) {
     k_zfwd_r<H><<<grid, 128, 0, p->stream>>>(d);
 }
 bool use_zreg(int Mz) {
-    static const int off = getenv("DNS_ZREG") ? (atoi(getenv("DNS_ZREG")) == 0) : 0;
-    return !off && (Mz == 24 || Mz == 36 || Mz == 48 || Mz == 72 || Mz == 96);
+    return dns_option("zreg") != 0 && (Mz == 24 || Mz == 36 || Mz == 48 || Mz == 72 || Mz == 96);
 }
 
-template <int R1, int R2> void zinv_launch(dns_plan* p, const double2* vin) {
+// dynamic shared memory attributes are set once per kernel and size, not per launch
+template <class K> void ensure_smem(K kern, size_t smem, size_t* have) {
+    if (*have >= smem) return;
+    cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    *have = smem;
+}
+
+template <int R1, int R2> void zinv_launch(dns_plan* p, const double2* vin, const double2* ein) {
     const DnsDev& d = p->d;
     const int ET = p->ETf, etlog = __builtin_ctz(ET), M = R1 * R2;
     const int nslots = 256 / ET;
@@ -380,10 +398,10 @@ template <int R1, int R2> void zinv_launch(dns_plan* p, const double2* vin) {
     while (NB > 1 && (size_t)(M + (size_t)NB * 2 * M * ET) * sizeof(double2) > 96 * 1024) --NB;
     const size_t smem = (size_t)(M + (size_t)NB * 2 * M * ET) * sizeof(double2);
     auto kern = k_zinv<R1, R2>;
-    cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
-    dim3 grid((unsigned)(d.Ni * ((d.nkx + NB - 1) / NB) * ((d.E + ET - 1) / ET)), 5);
-    kern<<<grid, 256, smem, p->stream>>>(d, vin, etlog, NB);
+    static size_t have = 0;
+    ensure_smem(kern, smem, &have);
+    dim3 grid((unsigned)(d.Ni * ((d.nkx + NB - 1) / NB) * ((d.E + ET - 1) / ET)), d.form == DNS_FORM_ROTATIONAL ? 6 : 5);
+    kern<<<grid, 256, smem, p->stream>>>(d, vin, ein, etlog, NB);
 }
 
 template <int R1, int R2> void zfwd_launch(dns_plan* p) {
@@ -395,8 +413,8 @@ template <int R1, int R2> void zfwd_launch(dns_plan* p) {
     while (NB > 1 && (size_t)(M + (size_t)NB * M * ET) * sizeof(double2) > 96 * 1024) --NB;
     const size_t smem = (size_t)(M + (size_t)NB * M * ET) * sizeof(double2);
     auto kern = k_zfwd<R1, R2>;
-    cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    static size_t have = 0;
+    ensure_smem(kern, smem, &have);
     dim3 grid((unsigned)(d.Ni * ((d.nkx + NB - 1) / NB) * ((d.E + ET - 1) / ET)), 3);
     kern<<<grid, 256, smem, p->stream>>>(d, etlog, NB);
 }
@@ -418,17 +436,17 @@ template <int R1, int R2> void zfwd_launch(dns_plan* p) {
         default: break;                                                   \
     }
 
-void launch_zinv(dns_plan* p, const double2* vin) {
+void launch_zinv(dns_plan* p, const double2* vin, const double2* ein) {
     if (use_zreg(p->d.Mz)) {
         switch (p->d.Mz) {
-            case 24: zinv_r_launch<12>(p, vin); return;
-            case 36: zinv_r_launch<18>(p, vin); return;
-            case 48: zinv_r_launch<24>(p, vin); return;
-            case 96: zinv_r4_launch<24>(p, vin); return;
-            default: zinv_r_launch<36>(p, vin); return;
+            case 24: zinv_r_launch<12>(p, vin, ein); return;
+            case 36: zinv_r_launch<18>(p, vin, ein); return;
+            case 48: zinv_r_launch<24>(p, vin, ein); return;
+            case 96: zinv_r4_launch<24>(p, vin, ein); return;
+            default: zinv_r_launch<36>(p, vin, ein); return;
         }
     }
-#define CALL(a, b) zinv_launch<a, b>(p, vin)
+#define CALL(a, b) zinv_launch<a, b>(p, vin, ein)
     DNS_FFT_DISPATCH(p->d.Mz, CALL)
 #undef CALL
 }

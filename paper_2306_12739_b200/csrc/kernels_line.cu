@@ -6,6 +6,9 @@
 //     holds exactly at interior rows for the u, w of Eq. 17-18),
 //   * forms the convective products u.grad u_i and the x-sums of u v, w v (Eq. 6-7) in registers,
 //   * returns (u.grad)u, (u.grad)v, (u.grad)w on the retained kx with 2 forward FFTs.
+// Rotational form (row f1, template parameter ROT): the 6 mixed fields u v w omega_x omega_y omega_z give the 6 physical
+// fields with 3 two-for-one inverse FFTs, H = omega x u and the x-sums of H_x, H_z are formed in registers, and the same
+// 2 forward FFTs return H on the retained kx.
 // Nothing in physical space ever reaches HBM.
 //
 // Thread mapping: a line is shared by SL "slots"; every slot owns R1 x-points of each physical field in registers.
@@ -68,10 +71,17 @@ template <int M, int NKX> __device__ __forceinline__ int pos_mode(int pos) {
 // Order in which the 8 mixed fields are consumed (sequence s -> field of I8: 0 u, 1 v, 2 w, 3 Du, 4 Dw, 5 uz, 6 vz,
 // 7 wz) by the six complex transforms Z = A + iB (A, B real in x):
 //   C = 0: (v, dv/dx)  1: (u, du/dx)  2: (w, dw/dx)  3: (Du, du/dz)  4: (Dw, dw/dz)  5: (dv/dz, -)
-__device__ __forceinline__ constexpr int seq_field(int s) {
-    return s == 0 ? 1 : s == 1 ? 0 : s == 2 ? 2 : s == 3 ? 3 : s == 4 ? 5 : s == 5 ? 4 : s == 6 ? 7 : 6;
+// Rotational form: sequence s = field s of I8 (u v w omega_x omega_y omega_z), three transforms of two fields each:
+//   C = 0: (u, v)  1: (w, omega_x)  2: (omega_y, omega_z)
+__device__ __forceinline__ constexpr int seq_field(int s, bool rot) {
+    return rot ? s : (s == 0 ? 1 : s == 1 ? 0 : s == 2 ? 2 : s == 3 ? 3 : s == 4 ? 5 : s == 5 ? 4 : s == 6 ? 7 : 6);
 }
-template <int C> struct LineSeq { static constexpr int sa = C < 3 ? C : (C == 3 ? 3 : (C == 4 ? 5 : 7)), two = (C == 3 || C == 4); };
+// first sequence of transform C and how its second field is made: 0 = a second stored field, 1 = i kx times the first,
+// 2 = none
+template <int C, bool ROT> struct LineSeq {
+    static constexpr int sa = ROT ? 2 * C : (C < 3 ? C : (C == 3 ? 3 : (C == 4 ? 5 : 7)));
+    static constexpr int mode = ROT ? 0 : ((C == 3 || C == 4) ? 0 : (C < 3 ? 1 : 2));
+};
 
 struct LineSmem {                     // byte offsets inside the dynamic shared memory of a CTA
     int kxs, group0, group_bytes, ring, buf, exch, red, bars, total;
@@ -98,13 +108,15 @@ __host__ __device__ inline LineSmem line_smem(int R1, int R2, int SL, int TPS, i
 
 // ------------------------------------------------------------------------------------------------ the kernel
 // grid = persistent CTAs ; block = NG groups of SL * TPS threads
-template <int R1, int R2, int SL, int TPS, int NG, int NST, int MINB>
+template <int R1, int R2, int SL, int TPS, int NG, int NST, int MINB, bool ROT>
 __global__ void __launch_bounds__(SL * TPS * NG, MINB) k_line(DnsDev d, int nitems) {
     constexpr int M = R1 * R2, NKX = M / 3, GT = SL * TPS;
+    constexpr int NSEQ = ROT ? 6 : 8;                        // input fields per item = sequence numbers of the ring
+    constexpr bool HALF = 2 * NST == NSEQ;                   // ring of half an item: every slot is used twice per item
     constexpr int PI = line_pitch(R2, TPS), PF = line_pitch(R1, TPS);
     constexpr int BUF = (R1 * PI > R2 * PF) ? R1 * PI : R2 * PF;
     constexpr int SLOT = NKX * TPS;                          // double2 per ring slot
-    static_assert(NST == 8 || NST == 4, "ring depth");
+    static_assert(NST == NSEQ || 2 * NST == NSEQ, "ring depth");
     extern __shared__ __align__(128) unsigned char smraw[];
     const LineSmem L = line_smem(R1, R2, SL, TPS, NG, NST);
     double* kxs = reinterpret_cast<double*>(smraw + L.kxs);
@@ -145,7 +157,7 @@ __global__ void __launch_bounds__(SL * TPS * NG, MINB) k_line(DnsDev d, int nite
         const uint32_t bytes = (uint32_t)(nl * NKX * ET * 16);
         uint64_t* bar = bars + (s % NST);
         mbar_arrive_expect_tx(bar, bytes);
-        bulk_g2s(ring + (s % NST) * SLOT, d.I8 + (size_t)seq_field(s) * fstride + off, bytes, bar);
+        bulk_g2s(ring + (s % NST) * SLOT, d.I8 + (size_t)seq_field(s, ROT) * fstride + off, bytes, bar);
     };
 
     int it = blockIdx.x * NG + grp;
@@ -174,18 +186,18 @@ __global__ void __launch_bounds__(SL * TPS * NG, MINB) k_line(DnsDev d, int nite
 
         // wait for sequence s of this item; refill slot after use with sequence s + NST (this or the next item)
         auto wait_seq = [&](int s) {
-            const uint32_t use = NST == 8 ? itc : 2 * itc + (s >= 4 ? 1 : 0);
+            const uint32_t use = HALF ? 2 * itc + (s >= NST ? 1 : 0) : itc;
             mbar_wait(bars + (s % NST), use & 1);
         };
         auto refill = [&](int s) {
             if (t != LEADER) return;
-            if (NST == 4 && s < 4) issue(it, s + 4);
-            else if (nxt < nitems) issue(nxt, NST == 8 ? s : s - 4);
+            if (HALF && s < NST) issue(it, s + NST);
+            else if (nxt < nitems) issue(nxt, HALF ? s - NST : s);
         };
 
 #define DNS_LINE_INV(C, BODY)                                                                         \
         {                                                                                             \
-            constexpr int sa = LineSeq<C>::sa, two = LineSeq<C>::two;                                 \
+            constexpr int sa = LineSeq<C, ROT>::sa, two = LineSeq<C, ROT>::mode == 0, ikx = LineSeq<C, ROT>::mode == 1; \
             wait_seq(sa);                                                                             \
             if (two) wait_seq(sa + 1);                                                                \
             double2* bufc = ((C) & 1) ? buf1 : buf0;                                                  \
@@ -207,7 +219,7 @@ __global__ void __launch_bounds__(SL * TPS * NG, MINB) k_line(DnsDev d, int nite
                             const double2 B = fb_s[n << etlog];                                       \
                             z = neg ? make_double2(A.x + B.y, B.x - A.y)                              \
                                     : (pos == 0 ? make_double2(A.x, B.x) : make_double2(A.x - B.y, A.y + B.x)); \
-                        } else if ((C) < 3) {                                                         \
+                        } else if (ikx) {                                                             \
                             const double kx = kxs[n];                                                 \
                             z = neg ? make_double2((1.0 + kx) * A.x, -(1.0 + kx) * A.y)               \
                                     : (pos == 0 ? make_double2(A.x, 0.0) : make_double2((1.0 - kx) * A.x, (1.0 - kx) * A.y)); \
@@ -241,16 +253,23 @@ __global__ void __launch_bounds__(SL * TPS * NG, MINB) k_line(DnsDev d, int nite
         // Z = A + iB:  Z(n) = A + iB, Z(0) = (Re A, Re B), Z(M - n) = conj(A) + i conj(B); with B = i kx A this is
         // Z(n) = (1 - kx) A, Z(M - n) = (1 + kx) conj(A).  Inverse transform by the swap identity: after the two
         // passes the first field is x.y and the second x.x.
-        DNS_LINE_INV(0, { v[k] = fa; Nv[k] = fb; })
-        DNS_LINE_INV(1, { u[k] = fa; Nu[k] = fa * fb; Nv[k] = fa * Nv[k] - v[k] * fb; suv += fa * v[k]; })
-        DNS_LINE_INV(2, { w[k] = fa; Nw[k] = u[k] * fb; swv += fa * v[k]; })
-        DNS_LINE_INV(3, { Nu[k] += v[k] * fa; Nu[k] += w[k] * fb; })
-        DNS_LINE_INV(4, { Nw[k] += v[k] * fa; Nw[k] += w[k] * fb; Nv[k] -= v[k] * fb; })
-        DNS_LINE_INV(5, { Nv[k] += w[k] * fa; })
+        if constexpr (!ROT) {
+            DNS_LINE_INV(0, { v[k] = fa; Nv[k] = fb; })
+            DNS_LINE_INV(1, { u[k] = fa; Nu[k] = fa * fb; Nv[k] = fa * Nv[k] - v[k] * fb; suv += fa * v[k]; })
+            DNS_LINE_INV(2, { w[k] = fa; Nw[k] = u[k] * fb; swv += fa * v[k]; })
+            DNS_LINE_INV(3, { Nu[k] += v[k] * fa; Nu[k] += w[k] * fb; })
+            DNS_LINE_INV(4, { Nw[k] += v[k] * fa; Nw[k] += w[k] * fb; Nv[k] -= v[k] * fb; })
+            DNS_LINE_INV(5, { Nv[k] += w[k] * fa; })
+        } else {
+            // H = omega x u: H_x = oy w - oz v, H_y = oz u - ox w, H_z = ox v - oy u; x-sums of H_x and H_z (Eq. 6-7)
+            DNS_LINE_INV(0, { u[k] = fa; v[k] = fb; })
+            DNS_LINE_INV(1, { w[k] = fa; Nv[k] = -(fb * fa); Nw[k] = fb * v[k]; })
+            DNS_LINE_INV(2, { Nu[k] = fa * w[k] - fb * v[k]; Nv[k] += fb * u[k]; Nw[k] -= fa * u[k]; suv += Nu[k]; swv += Nw[k]; })
+        }
 #undef DNS_LINE_INV
 
         // forward transforms of W1 = Nu + i Nv and W2 = Nw, factorisation (R2, R1): pass A on the registers
-        group_sync<GT>(grp);                                // pass B of transform 5 has finished reading buf1
+        group_sync<GT>(grp);                                // pass B of the last inverse transform has finished reading its buffer
         if (sl < R2) {
             double2 a1[R1], a2[R1];
 #pragma unroll
@@ -305,13 +324,15 @@ __global__ void __launch_bounds__(SL * TPS * NG, MINB) k_line(DnsDev d, int nite
     }
 }
 
-template <int R1, int R2, int SL, int TPS, int NG, int NST, int MINB> void line_launch(dns_plan* p) {
+template <int R1, int R2, int SL, int TPS, int NG, int NST8, int MINB, bool ROT> void line_launch_form(dns_plan* p) {
     const DnsDev& d = p->d;
+    constexpr int NST = ROT ? (NST8 * 3) / 4 : NST8;          // ring depth: a whole item (8 | 6 fields) or half of one
     const LineSmem L = line_smem(R1, R2, SL, TPS, NG, NST);
-    auto kern = k_line<R1, R2, SL, TPS, NG, NST, MINB>;
+    auto kern = k_line<R1, R2, SL, TPS, NG, NST, MINB, ROT>;
     const int LC = TPS >> d.etl;
     const int nitems = d.Ni * ((d.Mz + LC - 1) / LC) * d.ntl;
-    if (p->line_grid == 0) {
+    if (p->line_grid == 0 || p->line_grid_form != (int)ROT) {
+        p->line_grid_form = (int)ROT;
         cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, L.total);
         cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
         int nb = 0, nsm = 0, dev = 0;
@@ -325,6 +346,10 @@ template <int R1, int R2, int SL, int TPS, int NG, int NST, int MINB> void line_
     if (grid > p->line_grid) grid = p->line_grid;
     kern<<<grid, SL * TPS * NG, L.total, p->stream>>>(d, nitems);
 }
+template <int R1, int R2, int SL, int TPS, int NG, int NST8, int MINB> void line_launch(dns_plan* p) {
+    if (p->d.form == DNS_FORM_ROTATIONAL) line_launch_form<R1, R2, SL, TPS, NG, NST8, MINB, true>(p);
+    else line_launch_form<R1, R2, SL, TPS, NG, NST8, MINB, false>(p);
+}
 
 }  // namespace
 
@@ -334,7 +359,7 @@ template <int R1, int R2, int SL, int TPS, int NG, int NST, int MINB> void line_
 int dns_line_tps(int Mx, int E) {
     const bool small = (Mx == 18 || Mx == 24 || Mx == 36 || Mx == 48);
     int tps = E >= 16 ? 16 : (E >= 8 ? 8 : (small ? 4 : 8));
-    if (const char* s = getenv("DNS_LINE_TPS")) { int v = atoi(s); if (v == 8 || v == 16 || (v == 4 && small)) tps = v; }
+    { const int v = dns_option("line_tps"); if (v == 8 || v == 16 || (v == 4 && small)) tps = v; }
     return tps;
 }
 

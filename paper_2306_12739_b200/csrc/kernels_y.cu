@@ -127,6 +127,7 @@ __device__ void mean_body(const DnsDev& d, int stage, int derive_only, int tile,
     const bool eok = e < d.E;
     const int hi = stage == 0 ? 0 : 1;
     const double hdt = (stage == 0 ? 0.5 : 1.0) * d.dt;
+    const bool rot = d.form == DNS_FORM_ROTATIONAL;
     double* uvc = smm;                  // [Ny][8] RK-combined plane mean of u v
     double* wvc = uvc + Ny * 8;
     double* ru = wvc + Ny * 8;          // rhs / new profile U
@@ -164,7 +165,9 @@ __device__ void mean_body(const DnsDev& d, int stage, int derive_only, int tile,
         for (int i0 = 0; i0 < Ni; i0 += nrs) {                    // all lanes run every round (shuffles inside rowdot2)
             const int i = i0 + rs < Ni ? i0 + rs : Ni - 1;
             double su = 0.0, sw = 0.0;
-            rowdot2(d.Dfull + (size_t)(i + 1) * Ny, 1, Ny - 1, uvc, wvc, el, lane, su, sw);
+            // convective: S = d/dy of the plane mean of u v (Eq. 6-7, reading A9) ; rotational: S = plane mean of H_x itself
+            if (rot) { su = uvc[(i + 1) * 8 + el]; sw = wvc[(i + 1) * 8 + el]; }
+            else rowdot2(d.Dfull + (size_t)(i + 1) * Ny, 1, Ny - 1, uvc, wvc, el, lane, su, sw);
             const double ut = eok ? d.Ut[(size_t)(i + 1) * d.E + e] : 0.0, wt = eok ? d.Wt[(size_t)(i + 1) * d.E + e] : 0.0;
             if (i0 + rs < Ni) {
                 ru[i * 8 + el] = 2.0 * ut - hdt * su - 2.0 * d.bc[hi * Ni + i];
@@ -218,7 +221,7 @@ __device__ void mean_body(const DnsDev& d, int stage, int derive_only, int tile,
             const size_t gi = ((size_t)j * d.P) * d.E + e;
             d.uh[gi] = make_double2(Un[j * 8 + el], 0.0);
             d.wh[gi] = make_double2(Wn[j * 8 + el], 0.0);
-            d.duh[gi] = make_double2(du, 0.0);
+            d.duh[gi] = make_double2(rot ? -du : du, 0.0);      // rotational: omega_z = -dU/dy, omega_x = dW/dy at (0,0)
             d.dwh[gi] = make_double2(dw, 0.0);
         }
     }
@@ -266,6 +269,8 @@ k_ypair(DnsDev d, const __grid_constant__ CUtensorMap tmN, const __grid_constant
     const size_t rowstride = (size_t)d.P * d.E;             // complex elements between consecutive y rows
     const size_t pbase = (size_t)p * d.E + e0;              // + (row + 1) * rowstride + member
     double2* vout = stage == 2 ? d.vt : d.vs;
+    const bool rot = d.form == DNS_FORM_ROTATIONAL;
+    double2* eout = stage == 2 ? d.et : (rot ? d.es : nullptr);     // omega_y = eta is a transform input of omega x u
 
     // ---- stage the inputs: one TMA tile per field (box = Ni rows x ld doubles, landing in the padded panel layout;
     //      the 4 pad columns of every row are the first two members of the neighbouring tile: never used)
@@ -433,11 +438,11 @@ k_ypair(DnsDev d, const __grid_constant__ CUtensorMap tmN, const __grid_constant
             if (eokf(nt)) {
                 if (sok) {
                     vout[gS + 4 * nt] = make_double2(0.5 * (vS.x + vD.x), 0.5 * (vS.y + vD.y));
-                    if (stage == 2) d.et[gS + 4 * nt] = make_double2(0.5 * (eS.x + eD.x), 0.5 * (eS.y + eD.y));
+                    if (eout) eout[gS + 4 * nt] = make_double2(0.5 * (eS.x + eD.x), 0.5 * (eS.y + eD.y));
                 }
                 if (dok) {
                     vout[gD + 4 * nt] = make_double2(0.5 * (vS.x - vD.x), 0.5 * (vS.y - vD.y));
-                    if (stage == 2) d.et[gD + 4 * nt] = make_double2(0.5 * (eS.x - eD.x), 0.5 * (eS.y - eD.y));
+                    if (eout) eout[gD + 4 * nt] = make_double2(0.5 * (eS.x - eD.x), 0.5 * (eS.y - eD.y));
                 }
             }
         }
@@ -502,13 +507,25 @@ k_ypair(DnsDev d, const __grid_constant__ CUtensorMap tmN, const __grid_constant
 #pragma unroll
         for (int nt = 0; nt < NT; ++nt) {
             if (!eokf(nt)) continue;
+            double2 aS = make_double2(accS[nt][0], accS[nt][1]), aD = make_double2(accD[nt][0], accD[nt][1]);
+            double2 bS = make_double2(a2S[nt][0], a2S[nt][1]), bD = make_double2(a2D[nt][0], a2D[nt][1]);
+            if (rot) {
+                // omega_z = i kx v - du/dy, omega_x = dw/dy - i kz v (row f1): linear, so formed on the parity parts of
+                // v' (still in P0) and of the two derivatives
+                const double2 vS = sok ? ld2(P0 + offS + 8 * nt) : make_double2(0.0, 0.0);
+                const double2 vD = dok ? ld2(P0 + offD + 8 * nt) : make_double2(0.0, 0.0);
+                aS = make_double2(-kx * vS.y - aS.x, kx * vS.x - aS.y);
+                aD = make_double2(-kx * vD.y - aD.x, kx * vD.x - aD.y);
+                bS = make_double2(bS.x + kz * vS.y, bS.y - kz * vS.x);
+                bD = make_double2(bD.x + kz * vD.y, bD.y - kz * vD.x);
+            }
             if (sok) {
-                d.duh[gS + 4 * nt] = make_double2(0.5 * (accS[nt][0] + accD[nt][0]), 0.5 * (accS[nt][1] + accD[nt][1]));
-                d.dwh[gS + 4 * nt] = make_double2(0.5 * (a2S[nt][0] + a2D[nt][0]), 0.5 * (a2S[nt][1] + a2D[nt][1]));
+                d.duh[gS + 4 * nt] = make_double2(0.5 * (aS.x + aD.x), 0.5 * (aS.y + aD.y));
+                d.dwh[gS + 4 * nt] = make_double2(0.5 * (bS.x + bD.x), 0.5 * (bS.y + bD.y));
             }
             if (dok) {
-                d.duh[gD + 4 * nt] = make_double2(0.5 * (accS[nt][0] - accD[nt][0]), 0.5 * (accS[nt][1] - accD[nt][1]));
-                d.dwh[gD + 4 * nt] = make_double2(0.5 * (a2S[nt][0] - a2D[nt][0]), 0.5 * (a2S[nt][1] - a2D[nt][1]));
+                d.duh[gD + 4 * nt] = make_double2(0.5 * (aS.x - aD.x), 0.5 * (aS.y - aD.y));
+                d.dwh[gD + 4 * nt] = make_double2(0.5 * (bS.x - bD.x), 0.5 * (bS.y - bD.y));
             }
         }
     }
@@ -523,7 +540,7 @@ __global__ void __launch_bounds__(256) k_mean(DnsDev d, int stage, int derive_on
 
 // ------------------------------------------------------------------------------------------------ layout / IO
 // ABI [E][P][Ny] <-> internal [Ny][P][E]; grid = (P, ceil(E/32), ceil(Ny/32)), block = (32, 8)
-__global__ void k_abi_to_internal(const double2* __restrict__ src, double2* __restrict__ dst, int Ny, int P, int E) {
+__global__ void k_abi_to_internal(const double2* __restrict__ src, double2* __restrict__ dst, int Ny, int P, int E, int acc) {
     __shared__ double2 tile[32][33];
     const int p = blockIdx.x, e0 = blockIdx.y * 32, j0 = blockIdx.z * 32;
     for (int k = threadIdx.y; k < 32; k += 8) {
@@ -533,7 +550,11 @@ __global__ void k_abi_to_internal(const double2* __restrict__ src, double2* __re
     __syncthreads();
     for (int k = threadIdx.y; k < 32; k += 8) {
         const int j = j0 + k, e = e0 + threadIdx.x;
-        if (e < E && j < Ny) dst[((size_t)j * P + p) * E + e] = tile[threadIdx.x][k];
+        if (e < E && j < Ny) {
+            double2* o = dst + ((size_t)j * P + p) * E + e;
+            const double2 a = tile[threadIdx.x][k];
+            *o = acc ? make_double2(o->x + a.x, o->y + a.y) : a;
+        }
     }
 }
 __global__ void k_internal_to_abi(const double2* __restrict__ src, double2* __restrict__ dst, int Ny, int P, int E) {
@@ -594,18 +615,43 @@ __global__ void k_mean_out(DnsDev d, double* __restrict__ U, double* __restrict_
     }
 }
 
+// Sums over the retained modes of one wall-normal plane, per member, for the diagnostics: the 256 threads of a CTA are
+// EB member lanes x (256 / EB) mode slots; every slot walks the pairs p = slot, slot + nslot, ... and the slots are then
+// added in ascending order (fixed order: deterministic).  f(p, gi, acc) adds the contribution of pair p.
+template <int NS, class F> __device__ __forceinline__ void plane_mode_sums(const DnsDev& d, int j, int p0, double* sm, F f, double (&out)[NS], int e0, int EB) {
+    const int el = threadIdx.x % EB, slot = threadIdx.x / EB, nslot = blockDim.x / EB, e = e0 + el;
+    double acc[NS];
+#pragma unroll
+    for (int k = 0; k < NS; ++k) acc[k] = 0.0;
+    if (e < d.E)
+        for (int p = p0 + slot; p < d.P; p += nslot) f(p, ((size_t)j * d.P + p) * d.E + e, acc);
+#pragma unroll
+    for (int k = 0; k < NS; ++k) sm[(k * nslot + slot) * EB + el] = acc[k];
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < NS; ++k) {
+        double t = 0.0;
+        if (slot == 0)
+            for (int q = 0; q < nslot; ++q) t += sm[(k * nslot + q) * EB + el];
+        out[k] = t;
+    }
+    __syncthreads();
+}
+__device__ __forceinline__ int member_block(int E) { int b = 1; while (b < E && b < 256) b <<= 1; return b; }
+
 // diagnostics: energy partial sums per (j, e), then the per-member rows
-__global__ void k_diag_energy(DnsDev d, double* __restrict__ part) {
-    const int j = blockIdx.x;
-    for (int e = threadIdx.x; e < d.E; e += blockDim.x) {
-        double s = 0.0;
-        for (int p = 0; p < d.P; ++p) {
-            const size_t gi = ((size_t)j * d.P + p) * d.E + e;
+__global__ void __launch_bounds__(256) k_diag_energy(DnsDev d, double* __restrict__ part) {
+    __shared__ double sm[256];
+    const int j = blockIdx.x, EB = member_block(d.E);
+    for (int e0 = 0; e0 < d.E; e0 += EB) {
+        double s[1];
+        plane_mode_sums<1>(d, j, 0, sm, [&](int p, size_t gi, double* a) {
             const double2 u = d.uh[gi], v = d.vt[gi], w = d.wh[gi];
             const double cn = (p / d.nkz) == 0 ? 1.0 : 2.0;
-            s += cn * (u.x * u.x + u.y * u.y + v.x * v.x + v.y * v.y + w.x * w.x + w.y * w.y);
-        }
-        part[(size_t)j * d.E + e] = 0.25 * d.w[j] * s;
+            a[0] += cn * (u.x * u.x + u.y * u.y + v.x * v.x + v.y * v.y + w.x * w.x + w.y * w.y);
+        }, s, e0, EB);
+        const int e = e0 + threadIdx.x;
+        if (threadIdx.x < EB && e < d.E) part[(size_t)j * d.E + e] = 0.25 * d.w[j] * s[0];
     }
 }
 __global__ void k_diag_rows(DnsDev d, const double* __restrict__ part, double t) {
@@ -624,27 +670,67 @@ __global__ void k_diag_rows(DnsDev d, const double* __restrict__ part, double t)
 }
 
 // one-point statistics of the current state (row f4): Parseval sums over the retained modes, added to the running sums
-__global__ void k_stats(DnsDev d) {
-    const int j = blockIdx.x;
+__global__ void __launch_bounds__(256) k_stats(DnsDev d) {
+    __shared__ double sm[4 * 256];
+    const int j = blockIdx.x, EB = member_block(d.E);
     const size_t NE = (size_t)d.Ny * d.E;
-    for (int e = threadIdx.x; e < d.E; e += blockDim.x) {
-        double suu = 0.0, svv = 0.0, sww = 0.0, suv = 0.0;
-        for (int p = 1; p < d.P; ++p) {
-            const size_t gi = ((size_t)j * d.P + p) * d.E + e;
+    for (int e0 = 0; e0 < d.E; e0 += EB) {
+        double s[4];
+        plane_mode_sums<4>(d, j, 1, sm, [&](int p, size_t gi, double* a) {
             const double2 u = d.uh[gi], v = d.vt[gi], w = d.wh[gi];
             const double cn = (p / d.nkz) == 0 ? 1.0 : 2.0;      // the n = 0 plane stores both +-m, n > 0 stands for +-n
-            suu += cn * (u.x * u.x + u.y * u.y);
-            svv += cn * (v.x * v.x + v.y * v.y);
-            sww += cn * (w.x * w.x + w.y * w.y);
-            suv += cn * (u.x * v.x + u.y * v.y);
+            a[0] += cn * (u.x * u.x + u.y * u.y);
+            a[1] += cn * (v.x * v.x + v.y * v.y);
+            a[2] += cn * (w.x * w.x + w.y * w.y);
+            a[3] += cn * (u.x * v.x + u.y * v.y);
+        }, s, e0, EB);
+        const int e = e0 + threadIdx.x;
+        if (threadIdx.x < EB && e < d.E) {
+            const size_t o = (size_t)j * d.E + e;
+            d.stat[o] += d.Ut[o];
+            d.stat[NE + o] += s[0];
+            d.stat[2 * NE + o] += s[1];
+            d.stat[3 * NE + o] += s[2];
+            d.stat[4 * NE + o] += s[3];
         }
-        const size_t o = (size_t)j * d.E + e;
-        d.stat[o] += d.Ut[o];
-        d.stat[NE + o] += suu;
-        d.stat[2 * NE + o] += svv;
-        d.stat[3 * NE + o] += sww;
-        d.stat[4 * NE + o] += suv;
     }
+}
+
+// ------------------------------------------------------------------------------------------------ coupled ensemble (row f2)
+// the members share their streamwise-mean flow, which is forced by the Reynolds stresses averaged over
+// the members.  One warp per item = one run of E member values: the kx = 0 plane of the three components of the
+// nonlinear vector in spectral space ([3][Ni][nkz] items) and the per-z-line plane sums of the mean-flow sources
+// ([Ni][Mz] items).  phase 0: fixed-order sum over the members of this GPU -> d.ens (the exchange buffer);
+// phase 1: d.ens / E_total -> every member; phase 2: both at once (one GPU).
+__global__ void __launch_bounds__(256) k_ens(DnsDev d, int phase) {
+    const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    const int nN = 3 * d.Ni * d.nkz, nUV = d.Ni * d.Mz;
+    if (warp >= nN + nUV) return;
+    double2* run;
+    size_t slot;
+    if (warp < nN) {
+        const int f = warp / (d.Ni * d.nkz), r = warp % (d.Ni * d.nkz), j = r / d.nkz + 1, mi = r % d.nkz;
+        run = d.Nh + (size_t)f * d.S + ((size_t)j * d.P + mi) * d.E;
+        slot = ((size_t)f * d.Ny + j) * d.nkz + mi;
+    } else {
+        const int r = warp - nN, j = r / d.Mz + 1, q = r % d.Mz;
+        run = d.uvpart + ((size_t)j * d.Mz + q) * d.E;
+        slot = (size_t)3 * d.Ny * d.nkz + (size_t)j * d.Mz + q;
+    }
+    double2 t = make_double2(0.0, 0.0);
+    if (phase != 1) {
+        for (int e = lane; e < d.E; e += 32) { const double2 a = run[e]; t.x += a.x; t.y += a.y; }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {          // xor tree: the same order on every lane, every launch
+            t.x += __shfl_xor_sync(0xffffffffu, t.x, o);
+            t.y += __shfl_xor_sync(0xffffffffu, t.y, o);
+        }
+        if (phase == 0) { if (lane == 0) d.ens[slot] = t; return; }
+    } else {
+        t = d.ens[slot];
+    }
+    t.x *= d.invEtot; t.y *= d.invEtot;
+    for (int e = lane; e < d.E; e += 32) run[e] = t;
 }
 
 }  // namespace
@@ -691,8 +777,12 @@ template <int NT, int NWN> static void ypair_launch(dns_plan* p, int stage, int 
 #define LAUNCH(K)                                                                                     \
     {                                                                                                 \
         auto kern = k_ypair<NT, NWN, K>;                                                              \
-        cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);           \
-        cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared); \
+        static size_t attr_smem = 0;          /* the attributes are set once per instantiation and size, not per launch */ \
+        if (attr_smem < smem) {                                                                       \
+            cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);       \
+            cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared); \
+            attr_smem = smem;                                                                         \
+        }                                                                                             \
         const CUtensorMap* tm = reinterpret_cast<const CUtensorMap*>(p->tmaps);                       \
         kern<<<grid, 32 * KS2 * NWN, smem, p->stream>>>(d, tm[0], tm[1], tm[2], stage, derive_only); \
     }
@@ -719,14 +809,15 @@ void launch_ypair(dns_plan* p, int stage, int derive_only) {
 void launch_mean(dns_plan* p, int stage, int derive_only, cudaStream_t stream) {
     const DnsDev& d = p->d;
     const size_t smem = (size_t)6 * d.Ny * 8 * sizeof(double);
-    if (smem > 48 * 1024) cudaFuncSetAttribute(k_mean, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);   // Ny >= 129
+    static size_t attr_smem = 48 * 1024;
+    if (smem > attr_smem) { cudaFuncSetAttribute(k_mean, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr_smem = smem; }   // Ny >= 129
     k_mean<<<(d.E + 7) / 8, 256, smem, stream>>>(d, stage, derive_only);
 }
 
-void launch_abi_to_internal(dns_plan* p, const double2* src, double2* dst) {
+void launch_abi_to_internal(dns_plan* p, const double2* src, double2* dst, int accumulate) {
     const DnsDev& d = p->d;
     dim3 grid(d.P, (d.E + 31) / 32, (d.Ny + 31) / 32), block(32, 8);
-    k_abi_to_internal<<<grid, block, 0, p->stream>>>(src, dst, d.Ny, d.P, d.E);
+    k_abi_to_internal<<<grid, block, 0, p->stream>>>(src, dst, d.Ny, d.P, d.E, accumulate);
 }
 void launch_internal_to_abi(dns_plan* p, const double2* src, double2* dst) {
     const DnsDev& d = p->d;
@@ -740,7 +831,14 @@ void launch_mean_in(dns_plan* p, const double* U, const double* W) {
 void launch_mean_out(dns_plan* p, double* U, double* W) {
     k_mean_out<<<(p->d.E + 127) / 128, 128, 0, p->stream>>>(p->d, U, W);
 }
-void launch_stats(dns_plan* p) { k_stats<<<p->d.Ny, 128, 0, p->stream>>>(p->d); }
+void launch_stats(dns_plan* p) { k_stats<<<p->d.Ny, 256, 0, p->stream>>>(p->d); }
+
+size_t dns_ens_count(const DnsDev& d) { return 2 * ((size_t)3 * d.Ny * d.nkz + (size_t)d.Ny * d.Mz); }
+void launch_ens(dns_plan* p, int phase) {
+    const DnsDev& d = p->d;
+    const int nwarps = 3 * d.Ni * d.nkz + d.Ni * d.Mz;
+    k_ens<<<(nwarps + 7) / 8, 256, 0, p->stream>>>(d, phase);
+}
 void launch_diag(dns_plan* p, double t) {
     const DnsDev& d = p->d;
     double* part = d.diag + (size_t)d.E * 6;

@@ -21,6 +21,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <new>
 
 #include "dns_internal.h"
 
@@ -224,10 +225,13 @@ int dns_host_precompute(dns_plan* p) {
     const int Kp = d.Kp, Kh = (Ni + 1) / 2, Kho = Ni / 2;
     const size_t BB = (size_t)Kp * Kp;
     std::vector<double> mats((size_t)2 * nA * 6 * BB, 0.0);
-    int fail = 0;
+    int fail = 0, nomem = 0;
     const real dt = d.dt, Re = d.Re;
-#pragma omp parallel for schedule(dynamic, 1)
+    // an exception may not leave an OpenMP region (it would terminate the process, and nothing may abort across the ABI):
+    // allocation failures inside the loop body are caught per iteration and reported after the loop
+#pragma omp parallel for schedule(dynamic, 1) reduction(| : fail, nomem)
     for (int a = 1; a < nA; ++a) {
+        try {
         int n = a / d.nzh, m = a % d.nzh;
         // the stored kx, kz are fp64; alpha is formed from them exactly as the kernels do
         real alpha = (real)kx[n] * (real)kx[n] + (real)kz[m] * (real)kz[m];
@@ -242,7 +246,7 @@ int dns_host_precompute(dns_plan* p) {
         }
         LU = Del;
         std::vector<int> piv;
-        if (!lu_factor(LU, piv, Ni)) { fail = 1; continue; }
+        if (!lu_factor(LU, piv, Ni)) { fail |= 1; continue; }
         T = DelDel;
         lu_solve(LU, piv, T, Ni);                       // T = Delta^-1 Delta Delta (Eq. 12)
         Delinv.assign(NN, 0.0L);
@@ -254,7 +258,7 @@ int dns_host_precompute(dns_plan* p) {
             Mat A(NN), Sm(NN), Ainv, AD, Sinv;
             for (size_t i = 0; i < NN; ++i) { A[i] = -g * T[i]; Sm[i] = -g * Del[i]; }
             for (int i = 0; i < Ni; ++i) { A[(size_t)i * Ni + i] += 1.0L; Sm[(size_t)i * Ni + i] += 1.0L; }
-            if (!invert(A, Ainv, Ni) || !invert(Sm, Sinv, Ni)) { fail = 1; continue; }
+            if (!invert(A, Ainv, Ni) || !invert(Sm, Sinv, Ni)) { fail |= 1; continue; }
             matmul(Ainv, Delinv, AD, Ni);
             double* out = &mats[(((size_t)hi * nA + a) * 6) * BB];
             fold_block(Ainv, Ni, Kp, +1, Kh, out);
@@ -264,7 +268,11 @@ int dns_host_precompute(dns_plan* p) {
             fold_block(Sinv, Ni, Kp, +1, Kh, out + 4 * BB);
             fold_block(Sinv, Ni, Kp, -1, Kho, out + 5 * BB);
         }
+        } catch (const std::bad_alloc&) {
+            nomem |= 1;
+        }
     }
+    if (nomem) return DNS_ENOMEM;
     if (fail) return DNS_EINVAL;
     // ---- mean-flow operators (Eq. 14-15; boundary columns moved to the rhs)
     std::vector<double> S0inv(2 * NN), bc(2 * Ni), Ugam(2 * Ni);

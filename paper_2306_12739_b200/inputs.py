@@ -175,6 +175,49 @@ def make_state(cfg: Config, members=None):
     return {"vhat": vhat, "etahat": ehat, "U00": U00, "W00": W00, "rms": rms, "sha256": h.hexdigest()}
 
 
+def broadband_member_state(cfg: Config, e: int, amp: float = 0.01):
+    """A second, rough family of inputs for parity tests at the full sizes: EVERY retained pair (n, m) != (0, 0) carries
+    energy, amplitude amp (1 + n^2 + m^2)^(-5/6) (a k^(-5/3)-like spectrum), and the wall-normal profiles are Chebyshev
+    series of degree Ny - 5 with slowly decaying random coefficients c_k ~ N(0,1)/sqrt(1 + k) under the no-slip
+    envelopes:  vhat = (1-y^2)^2 sum c_k T_k(y),  etahat = (1-y^2) sum c'_k T_k(y)  (Eq. 8).  No scaling by
+    the energy (that would need the method's arithmetic): amp sets the level directly."""
+    Nx, Ny, Nz = cfg.Nx, cfg.Ny, cfg.Nz
+    nkx, nkz = Nx // 2, Nz - 1
+    y = grid_y(Ny)
+    rng = np.random.default_rng([20230612, 100 + cfg.cid, e])
+    deg = Ny - 5
+    decay = 1.0 / np.sqrt(1.0 + np.arange(deg + 1))
+    T = np.cos(np.outer(np.arange(deg + 1), np.arccos(np.clip(y, -1.0, 1.0))))     # T_k(y_j)
+    mo = m_of_index(Nz)
+    a = amp * (1.0 + np.arange(nkx)[:, None] ** 2 + mo[None, :] ** 2) ** (-5.0 / 6.0)
+    cv = (rng.standard_normal((nkx, nkz, deg + 1)) + 1j * rng.standard_normal((nkx, nkz, deg + 1))) * decay
+    ce = (rng.standard_normal((nkx, nkz, deg + 1)) + 1j * rng.standard_normal((nkx, nkz, deg + 1))) * decay
+    vhat = a[:, :, None] * (cv @ T) * ((1.0 - y * y) ** 2)[None, None, :]
+    ehat = a[:, :, None] * (ce @ T) * (1.0 - y * y)[None, None, :]
+    vhat[0, 0] = 0.0
+    ehat[0, 0] = 0.0
+    for i, m in enumerate(mo):                     # real field: the m < 0 half of the n = 0 plane mirrors m > 0
+        if m < 0:
+            vhat[0, i] = np.conj(vhat[0, m_index(-int(m), Nz)])
+            ehat[0, i] = np.conj(ehat[0, m_index(-int(m), Nz)])
+    for f in (vhat, ehat):
+        f[..., 0] = 0.0
+        f[..., -1] = 0.0
+    return vhat, ehat, laminar_profile(cfg, y), np.zeros(Ny)
+
+
+def make_broadband_state(cfg: Config, members=None, amp: float = 0.01):
+    members = list(range(cfg.E) if members is None else members)
+    nkx, nkz = cfg.Nx // 2, cfg.Nz - 1
+    vhat = np.empty((len(members), nkx, nkz, cfg.Ny), np.complex128)
+    ehat = np.empty_like(vhat)
+    U00 = np.empty((len(members), cfg.Ny))
+    W00 = np.empty_like(U00)
+    for i, e in enumerate(members):
+        vhat[i], ehat[i], U00[i], W00[i] = broadband_member_state(cfg, e, amp)
+    return {"vhat": vhat, "etahat": ehat, "U00": U00, "W00": W00}
+
+
 def plan_args(cfg: Config, E=None):
     """Positional arguments of dns_plan_create / the oracle constructor."""
     return (cfg.Nx, cfg.Ny, cfg.Nz, cfg.E if E is None else int(E), cfg.Re, cfg.Lx, cfg.Lz, cfg.dt, cfg.flow)

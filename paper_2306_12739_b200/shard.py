@@ -31,6 +31,14 @@ def gather_rows(local_rows: np.ndarray, E: int, ncols: int):
     return np.concatenate([o[:c].cpu().numpy() for o, c in zip(out, counts)], axis=0)
 
 
+def allreduce_sum_(t) -> None:
+    """In-place sum over all ranks of a torch tensor (the exchange step of a coupled ensemble sharded over GPUs,
+    SURVEY.md 8(f) row f2): NCCL on the tensor's CUDA stream order, gloo for CPU tensors."""
+    import torch.distributed as dist
+
+    dist.all_reduce(t, op=dist.ReduceOp.SUM)
+
+
 def max_over_ranks(x: float) -> float:
     import torch
     import torch.distributed as dist
