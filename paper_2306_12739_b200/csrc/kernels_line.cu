@@ -151,13 +151,18 @@ __global__ void __launch_bounds__(SL * TPS * NG, MINB) k_line(DnsDev d, int nite
         nl = d.Mz - qg * LC < LC ? d.Mz - qg * LC : LC;
         return ((((size_t)jj * d.Mz + (size_t)qg * LC) * ntile + te) * NKX) << etlog;
     };
+    // lines q, q+1, .. of one member tile are contiguous in the mixed arrays only when there is a single tile
+    const size_t gline = ((size_t)ntile * NKX) << etlog;      // elements between consecutive z lines of one tile
     auto issue = [&](int it, int s) {                         // leader only: fetch sequence s of item it
         int nl;
         const size_t off = item_off(it, nl);
         const uint32_t bytes = (uint32_t)(nl * NKX * ET * 16);
         uint64_t* bar = bars + (s % NST);
         mbar_arrive_expect_tx(bar, bytes);
-        bulk_g2s(ring + (s % NST) * SLOT, d.I8 + (size_t)seq_field(s, ROT) * fstride + off, bytes, bar);
+        const double2* src = d.I8 + (size_t)seq_field(s, ROT) * fstride + off;
+        if (ntile == 1) bulk_g2s(ring + (s % NST) * SLOT, src, bytes, bar);
+        else
+            for (int l = 0; l < nl; ++l) bulk_g2s(ring + (s % NST) * SLOT + l * NKX * ET, src + l * gline, bytes / nl, bar);
     };
 
     int it = blockIdx.x * NG + grp;
@@ -300,7 +305,7 @@ __global__ void __launch_bounds__(SL * TPS * NG, MINB) k_line(DnsDev d, int nite
         }
         group_sync<GT>(grp);
         if (sl < R1 && lok) {
-            double2* dst = d.I3 + ioff + lidx;
+            double2* dst = d.I3 + ioff + (size_t)lc * gline + el;
 #pragma unroll
             for (int k = 0; k < R2; ++k) {
                 const int lo = R1 * k;
@@ -372,8 +377,18 @@ template <int R1, int R2, int SL> static void line_launch_tps(dns_plan* p) {
         case 8: line_launch<R1, R2, SL, 8, SL == 8 ? 2 : 1, big ? 4 : 8, SL == 8 ? 3 : (big ? 3 : 4)>(p); break;
         default:
             // small family: ring depth 4 measured best on config 2 (155 -> 141 us); 3 CTAs per SM without spills
-            if constexpr (SL == 8) line_launch<R1, R2, SL, 16, 1, 4, 3>(p);
-            else line_launch<R1, R2, SL, 16, 1, 4, 2>(p);
+            // ring depth: half an item for the convective form (measured best on config 2: 155 -> 141 us; a whole item
+            // changes nothing), a whole item for the rotational form, where three transforms drain six fields too fast
+            // for a half ring (config 4: 1381 -> 1281 us, config 2: 109 -> 96 us).  Option "line_ring": 0 half, 1 whole.
+            {
+                const int ring = dns_option("line_ring");
+                const bool whole = !big && (ring < 0 ? p->d.form == DNS_FORM_ROTATIONAL : ring == 1);
+                constexpr int MB = SL == 8 ? 3 : 2;
+                if constexpr (!big) {
+                    if (whole) { line_launch<R1, R2, SL, 16, 1, 8, MB>(p); break; }
+                }
+                line_launch<R1, R2, SL, 16, 1, 4, MB>(p);
+            }
             break;
     }
 }
@@ -386,7 +401,13 @@ void launch_line(dns_plan* p) {
         case 36: line_launch_tps<6, 6, 8>(p); break;
         case 48: line_launch_tps<6, 8, 8>(p); break;
         case 54: line_launch_tps<6, 9, 12>(p); break;
-        case 72: line_launch_tps<6, 12, 12>(p); break;
+        case 72:
+            // option "line_alt" = 1: 72 = 8 x 9 on 9 slots of one warp each (32 lanes = 2 lines x 16 members): 8 of 9 slots
+            // work in the first pass and all 9 in the second, against 6 of 12 with 6 x 12 -- but only 9 warps per SM fit
+            // (140 KB, 168 registers); measured on config 4: 2128 us against 2010 us, so it is not the default
+            if (p->line_tps == 16 && dns_option("line_alt") == 1) line_launch<8, 9, 9, 32, 1, 4, 1>(p);
+            else line_launch_tps<6, 12, 12>(p);
+            break;
         case 81: line_launch_tps<9, 9, 12>(p); break;
         case 96: line_launch_tps<8, 12, 12>(p); break;
         case 108: line_launch_tps<9, 12, 12>(p); break;
