@@ -163,6 +163,41 @@ int dns_stats_reset(dns_plan* plan);
 int dns_stats_accumulate(dns_plan* plan);
 int dns_stats_get(dns_plan* plan, double* out, long long* nsamples);
 
+/* ---- Linearised forward / adjoint ensemble (section 4.1.1, Appendix B :390-417) ----
+ * E = nmodes * Eg disturbance vectors advanced at once.  Vector e = g Eg + i has the single streamwise wavenumber
+ * kx = 2 pi n_list[g] / Lx ("we may specify the streamwise wavenumber of each disturbance") and no mean flow, so only
+ * Eq. 12-13 are solved, with the precomputed single-kx operators of that vector, which also serve the adjoint.
+ * The base flow (U, V, W)(y, z) is the frozen streamwise-mean (kx = 0) part of a DNS state (Fig. 7(a)).
+ *   forward (Eq. B.2):  d u'/dt     = -[(U.grad)u' + (u'.grad)U] - grad p' + (1/Re) Lap u'
+ *   adjoint (Eq. B.5):  d lam/d tau = +[(U.grad)lam + U_i grad lam_i] - grad b + (1/Re) Lap lam,  tau = T - t (reversed time)
+ * stepped with the CN/RK3 scheme of PAPER.md:120-126 at dt_lin = t_f dt (time-step factor t_f, :315).  Energy inner product
+ * (Eq. B.1) <a,b> = 1/(2V) int conj(a).b dV.  Layout: vhat, etahat [E][nkz][Ny] complex128 (m in FFT order, y ascending).
+ *
+ * dns_lin_plan_create  -- as dns_plan_create (same grid limits); n_list[nmodes] with 1 <= n < Nx/2; Eg members per mode;
+ *                         dt_lin the step of the linear problem.  Workspace, binding and destruction:
+ *                         dns_plan_workspace_bytes, dns_plan_bind, dns_plan_destroy.  Errors: DNS_EINVAL, DNS_ENOMEM, DNS_ECUDA.
+ * dns_lin_set_base     -- base flow := streamwise-mean flow of member `member` of the CURRENT state of a DNS plan with the
+ *                         same grid and box, in the convective form (its transform scratch is overwritten; synchronises that
+ *                         plan's stream).  Errors: DNS_EINVAL (mismatch, rotational form, bad member), DNS_ESTATE, DNS_ECUDA.
+ * dns_lin_set_state / dns_lin_get_state -- host or device pointers; wall rows are set to 0; get synchronises.
+ * dns_lin_step         -- enqueue nsteps steps of the forward (adjoint = 0) or adjoint (adjoint = 1) equations.
+ * dns_lin_energy       -- out[E] = <q_e, q_e> (host or device); synchronises.
+ * dns_lin_orthonormalise -- modified Gram-Schmidt in member order within every kx group, energy inner product (:417).
+ * dns_lin_optimals     -- the power iteration of :417: orthonormalise; niter times { nsteps forward, record the gains
+ *                         E(T_opt)/E(0), nsteps adjoint from the forward final state, orthonormalise }; gains[E] (host or
+ *                         device) are those of the last forward leg.  T_opt = nsteps dt_lin.  Synchronises.
+ * All: DNS_EINVAL for a non-linear plan or bad arguments, DNS_ESTATE before bind / set_base / set_state, DNS_ECUDA. */
+int dns_lin_plan_create(dns_plan** out, int Nx, int Ny, int Nz, int nmodes, const int* n_list, int Eg, double Re, double Lx,
+                        double Lz, double dt_lin);
+int dns_lin_set_base(dns_plan* lin, dns_plan* dns, int member);
+int dns_lin_set_state(dns_plan* lin, const double* vhat, const double* etahat);
+int dns_lin_get_state(dns_plan* lin, double* vhat, double* etahat);
+int dns_lin_step(dns_plan* lin, int nsteps, int adjoint);
+int dns_lin_energy(dns_plan* lin, double* out);
+int dns_lin_orthonormalise(dns_plan* lin);
+int dns_lin_optimals(dns_plan* lin, int nsteps, int niter, double* gains);
+int dns_lin_launches_per_step(const dns_plan* lin);
+
 /* Number of kernel launches one dns_step(1) enqueues (for bench.py's gpu_launches). */
 int dns_launches_per_step(const dns_plan* plan);
 

@@ -11,8 +11,8 @@ flow (U, V, W)(y, z) is a frozen streamwise-mean flow, i.e. the kx = 0 part of a
   forward  (B.2):  d u'/dt     = -[(U.grad)u' + (u'.grad)U] - grad p' + (1/Re) Lap u'
   adjoint  (B.5):  d lam/d tau = +[(U.grad)lam + U_i grad lam_i] - grad b + (1/Re) Lap lam,   tau = T - t
 Both have the form of the momentum equation with a "nonlinear vector" N that is linear in the disturbance, so F, G of
-Eq. 4-5 and the CN/RK3 stages of Eq. 11-13 are reused unchanged through oracle.dns_oracle.Oracle,
-whose stage() and operators are pinned by tests/test_oracle_pins.py ("The matrices are also valid for the adjoint
+Eq. 4-5 and the CN/RK3 stages of Eq. 11-13 are reused unchanged, with the operators and LU factors
+of oracle.dns_oracle.Oracle, which are pinned by tests/test_oracle_pins.py ("The matrices are also valid for the adjoint
 equations", :304).  Products are formed on the 3/2-padded z grid (x is analytic: d/dx = i kx).
 Energy inner product (B.1): <a, b> = 1/(2V) int conj(a).b dV over the pair of modes +-kx
                                    = (1/2) sum_m sum_j w_j (conj(u_a) u_b + conj(v_a) v_b + conj(w_a) w_b).
@@ -127,19 +127,24 @@ class LinearEnsemble:
 
     # ---------------------------------------------------------------- CN/RK3 step of Eq. 12-13
     def _stage(self, v_t, eta_t, h, F, G):
-        """Oracle.stage on full-shaped arrays that are zero outside the member's own kx row."""
+        """Eq. 12-13 for every member and every kz of its own kx row, with the LU factors of the pinned Oracle (the same
+        statements as Oracle.stage, restricted to the rows that are not identically zero):
+          [I - g T] v' = [I + g T] v_t - h dt Delta^-1 F          (Eq. 12)
+          [I - g Delta] eta' = [I + g Delta] eta_t - h dt G        (Eq. 13)"""
+        import scipy.linalg as sla
         o = self.o
-        shp = (self.E, o.nkx, o.nkz)
-        vt, et = np.zeros(shp + (o.Ny,), np.complex128), np.zeros(shp + (o.Ny,), np.complex128)
-        Ff, Gf = np.zeros(shp + (o.Ni,), np.complex128), np.zeros(shp + (o.Ni,), np.complex128)
+        hdt = h * o.dt
+        v_n, eta_n = np.zeros_like(v_t), np.zeros_like(eta_t)
         for e in range(self.E):
             n = self.n_of[e]
-            vt[e, n], et[e, n], Ff[e, n], Gf[e, n] = v_t[e], eta_t[e], F[e], G[e]
-        Z = np.zeros((self.E, o.Ny))
-        o.Qstar = np.zeros(self.E)                                          # the disturbances carry no mean flow (:304)
-        vn, en, _, _, _ = o.stage(vt, et, Z, Z, h, Ff, Gf, Z, Z)
-        return (np.stack([vn[e, self.n_of[e]] for e in range(self.E)]),
-                np.stack([en[e, self.n_of[e]] for e in range(self.E)]))
+            for m in range(o.nkz):
+                a = o.alpha[n, m]
+                Lf, luDel = o.lu[(h, a)], o.ops[a][2]
+                rhs = Lf["B"] @ v_t[e, m, 1:-1] - hdt * sla.lu_solve(luDel, F[e, m])
+                v_n[e, m, 1:-1] = sla.lu_solve(Lf["A"], rhs)
+                rhs = Lf["Sp"] @ eta_t[e, m, 1:-1] - hdt * G[e, m]
+                eta_n[e, m, 1:-1] = sla.lu_solve(Lf["Sm"], rhs)
+        return v_n, eta_n
 
     def _forcing_all(self, adjoint):
         FG = [self.forcing(e, adjoint) for e in range(self.E)]

@@ -28,6 +28,8 @@ EXPORTS = ("dns_plan_create", "dns_plan_set_form", "dns_plan_set_coupling", "dns
            "dns_plan_workspace_bytes", "dns_plan_bind", "dns_set_state", "dns_step",
            "dns_step_profile", "dns_get_state", "dns_diagnostics", "dns_stats_reset", "dns_stats_accumulate", "dns_stats_get",
            "dns_launches_per_step", "dns_plan_destroy", "dns_strerror",
+           "dns_lin_plan_create", "dns_lin_set_base", "dns_lin_set_state", "dns_lin_get_state", "dns_lin_step",
+           "dns_lin_energy", "dns_lin_orthonormalise", "dns_lin_optimals", "dns_lin_launches_per_step",
            "dns_debug_fetch", "dns_debug_stage", "dns_debug_set_option", "dns_debug_fp64_peak")
 EXCHANGE_FN = ctypes.CFUNCTYPE(ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p)
 
@@ -87,6 +89,24 @@ def lib():
         L.dns_plan_set_exchange.restype = i
         L.dns_add_increment.argtypes = [vp, dp, dp]
         L.dns_add_increment.restype = i
+        L.dns_lin_plan_create.argtypes = [ctypes.POINTER(vp), i, i, i, i, ctypes.POINTER(i), i, d, d, d, d]
+        L.dns_lin_plan_create.restype = i
+        L.dns_lin_set_base.argtypes = [vp, vp, i]
+        L.dns_lin_set_base.restype = i
+        L.dns_lin_set_state.argtypes = [vp, dp, dp]
+        L.dns_lin_set_state.restype = i
+        L.dns_lin_get_state.argtypes = [vp, dp, dp]
+        L.dns_lin_get_state.restype = i
+        L.dns_lin_step.argtypes = [vp, i, i]
+        L.dns_lin_step.restype = i
+        L.dns_lin_energy.argtypes = [vp, dp]
+        L.dns_lin_energy.restype = i
+        L.dns_lin_orthonormalise.argtypes = [vp]
+        L.dns_lin_orthonormalise.restype = i
+        L.dns_lin_optimals.argtypes = [vp, i, i, dp]
+        L.dns_lin_optimals.restype = i
+        L.dns_lin_launches_per_step.argtypes = [vp]
+        L.dns_lin_launches_per_step.restype = i
         L.dns_debug_set_option.argtypes = [ctypes.c_char_p, i]
         L.dns_debug_set_option.restype = i
         L.dns_debug_fp64_peak.argtypes = [i, d, ctypes.POINTER(d)]
@@ -141,6 +161,46 @@ def dns_debug_fp64_peak(kind: int, seconds: float):
     t = ctypes.c_double(0.0)
     st = lib().dns_debug_fp64_peak(int(kind), float(seconds), ctypes.byref(t))
     return st, float(t.value)
+
+
+def dns_lin_plan_create(Nx, Ny, Nz, n_list, Eg, Re, Lx, Lz, dt_lin):
+    h = ctypes.c_void_p()
+    arr = (ctypes.c_int * len(n_list))(*[int(n) for n in n_list])
+    st = lib().dns_lin_plan_create(ctypes.byref(h), int(Nx), int(Ny), int(Nz), len(n_list), arr, int(Eg), float(Re),
+                                   float(Lx), float(Lz), float(dt_lin))
+    return st, h
+
+
+def dns_lin_set_base(h, dns_h, member: int) -> int:
+    return lib().dns_lin_set_base(h, dns_h, int(member))
+
+
+def dns_lin_set_state(h, vhat, etahat) -> int:
+    return lib().dns_lin_set_state(h, _ptr(vhat), _ptr(etahat))
+
+
+def dns_lin_get_state(h, vhat, etahat) -> int:
+    return lib().dns_lin_get_state(h, _ptr(vhat), _ptr(etahat))
+
+
+def dns_lin_step(h, nsteps: int, adjoint: int) -> int:
+    return lib().dns_lin_step(h, int(nsteps), int(adjoint))
+
+
+def dns_lin_energy(h, out) -> int:
+    return lib().dns_lin_energy(h, _ptr(out))
+
+
+def dns_lin_orthonormalise(h) -> int:
+    return lib().dns_lin_orthonormalise(h)
+
+
+def dns_lin_optimals(h, nsteps: int, niter: int, gains) -> int:
+    return lib().dns_lin_optimals(h, int(nsteps), int(niter), _ptr(gains))
+
+
+def dns_lin_launches_per_step(h) -> int:
+    return lib().dns_lin_launches_per_step(h)
 
 
 def dns_plan_workspace_bytes(h) -> int:
@@ -326,6 +386,80 @@ class Plan:
 
     def launches_per_step(self):
         return dns_launches_per_step(self.h)
+
+    def close(self):
+        if self.h is not None:
+            dns_plan_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+class LinPlan:
+    """dns_lin_plan_create + a torch-allocated workspace bound on torch's current stream (linearised forward / adjoint
+    ensemble).  E = len(n_list) * Eg members, [E][nkz][Ny] complex128."""
+
+    def __init__(self, Nx, Ny, Nz, n_list, Eg, Re, Lx, Lz, dt_lin, device="cuda:0"):
+        import torch
+
+        self.E = len(n_list) * int(Eg)
+        self.shape = (self.E, int(Nz) - 1, int(Ny))
+        self.device = torch.device(device)
+        self.h = None
+        if not torch.cuda.is_available():
+            raise DnsError(DNS_ECUDA, "LinPlan (no CUDA device; this library has no CPU path)")
+        torch.cuda.set_device(self.device)
+        st, h = dns_lin_plan_create(Nx, Ny, Nz, n_list, Eg, Re, Lx, Lz, dt_lin)
+        if st != DNS_OK:
+            raise DnsError(st, "dns_lin_plan_create")
+        self.h = h
+        nbytes = dns_plan_workspace_bytes(h)
+        self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        base = (self.workspace.data_ptr() + 255) & ~255
+        self.stream = torch.cuda.current_stream(self.device)
+        st = dns_plan_bind(h, base, nbytes, self.stream.cuda_stream)
+        if st != DNS_OK:
+            raise DnsError(st, "dns_plan_bind")
+        self.workspace_bytes = nbytes
+
+    def _chk(self, st, where):
+        if st != DNS_OK:
+            raise DnsError(st, where)
+
+    def set_base(self, dns_plan, member=0):
+        self._chk(dns_lin_set_base(self.h, dns_plan.h, member), "dns_lin_set_base")
+
+    def set_state(self, vhat, etahat):
+        if isinstance(vhat, np.ndarray):
+            vhat = np.ascontiguousarray(vhat, dtype=np.complex128)
+            etahat = np.ascontiguousarray(etahat, dtype=np.complex128)
+            assert vhat.shape == self.shape and etahat.shape == self.shape
+        self._chk(dns_lin_set_state(self.h, vhat, etahat), "dns_lin_set_state")
+
+    def get_state(self):
+        out = (np.empty(self.shape, np.complex128), np.empty(self.shape, np.complex128))
+        self._chk(dns_lin_get_state(self.h, *out), "dns_lin_get_state")
+        return out
+
+    def step(self, nsteps=1, adjoint=False):
+        self._chk(dns_lin_step(self.h, nsteps, 1 if adjoint else 0), "dns_lin_step")
+
+    def energy(self):
+        out = np.empty(self.E)
+        self._chk(dns_lin_energy(self.h, out), "dns_lin_energy")
+        return out
+
+    def orthonormalise(self):
+        self._chk(dns_lin_orthonormalise(self.h), "dns_lin_orthonormalise")
+
+    def optimals(self, nsteps, niter):
+        out = np.empty(self.E)
+        self._chk(dns_lin_optimals(self.h, nsteps, niter, out), "dns_lin_optimals")
+        return out
 
     def close(self):
         if self.h is not None:

@@ -8,7 +8,8 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libdns_b200.so")
-SOURCES = ["api.cu", "plan.cu", "kernels_fft.cu", "kernels_line.cu", "kernels_y.cu", "peak_fp64.cu"]
+SOURCES = ["api.cu", "plan.cu", "kernels_fft.cu", "kernels_line.cu", "kernels_y.cu", "peak_fp64.cu",
+           "kernels_lin.cu", "api_lin.cu"]
 HEADERS = ["dns_internal.h", "fft_codelets.cuh", "fft_consts.h", os.path.join("..", "..", "include", "dns.h"),
            os.path.join("..", "..", "include", "dns_debug.h")]
 NVCC_FLAGS = [

@@ -50,6 +50,8 @@ size_t carve_workspace(dns_plan* p, void* base) {
     d.uvpart = c.take<double2>((size_t)d.Ny * d.Mz * d.E);
     d.uvc0 = c.take<double2>(NE);
     d.ens = c.take<double2>(dns_ens_count(d) / 2);
+    d.base = c.take<double>(d.lin ? (size_t)9 * d.Ny * d.Mz : 1);
+    d.lin_scr = c.take<double>(d.lin ? (size_t)2 * d.E + (size_t)d.Ny * d.E : 1);
     d.Ut = c.take<double>(NE);  d.Wt = c.take<double>(NE);  d.Us = c.take<double>(NE);  d.Ws = c.take<double>(NE);
     d.gamma = c.take<double>(d.E);  d.Qstar = c.take<double>(d.E);
     d.diag = c.take<double>((size_t)d.E * 6 + NE);
@@ -155,8 +157,11 @@ const char* dns_strerror(int s) {
     }
 }
 
-int dns_plan_create(dns_plan** out, int Nx, int Ny, int Nz, int E, double Re, double Lx, double Lz, double dt,
-                    int flow) {
+}  // extern "C"
+
+// dns_plan_create and dns_lin_plan_create: nmodes = 0 for a DNS plan; otherwise E = nmodes * Eg single-kx members
+int dns_create_common(dns_plan** out, int Nx, int Ny, int Nz, int E, double Re, double Lx, double Lz, double dt, int flow,
+                      int nmodes, const int* n_list, int Eg) {
     if (!out) return DNS_EINVAL;
     *out = nullptr;
     if (Nx < 2 || Nz < 4 || (Nx & 1) || (Nz & 1)) return DNS_EINVAL;
@@ -174,12 +179,19 @@ int dns_plan_create(dns_plan** out, int Nx, int Ny, int Nz, int E, double Re, do
     if (!p) return DNS_ENOMEM;
     DnsDev& d = p->d;
     d.Nx = Nx; d.Ny = Ny; d.Nz = Nz; d.E = E; d.Mx = Mx; d.Mz = Mz;
-    d.nkx = Nx / 2; d.nkz = Nz - 1; d.nzh = Nz / 2; d.P = d.nkx * d.nkz; d.Ni = Ny - 2; d.flow = flow;
-    d.dt = dt; d.Re = Re; d.Uw = flow == DNS_COUETTE ? 1.0 : 0.0; d.invMxMz = 1.0 / ((double)Mx * Mz);
+    d.nkxm = Nx / 2; d.lin = nmodes > 0; d.nmodes = nmodes; d.Eg = Eg;
+    d.nkx = d.lin ? 1 : Nx / 2; d.nkz = Nz - 1; d.nzh = Nz / 2; d.P = d.nkx * d.nkz; d.Ni = Ny - 2; d.flow = flow;
+    if (d.lin) {
+        for (int g = 0; g < nmodes; ++g)
+            if (n_list[g] < 1 || n_list[g] >= d.nkxm) { delete p; return DNS_EINVAL; }
+        p->nlist_host.assign(n_list, n_list + nmodes);
+    }
+    d.dt = dt; d.Re = Re; d.Uw = flow == DNS_COUETTE ? 1.0 : 0.0;
+    d.invMxMz = d.lin ? 1.0 / Mz : 1.0 / ((double)Mx * Mz);       // single-kx members: x is analytic, only z is transformed
     d.form = DNS_FORM_CONVECTIVE; d.coupling = DNS_COUPLING_NONE; d.invEtot = 1.0 / E;
     d.S = (size_t)Ny * d.P * E;
     {
-        const int tps = dns_line_tps(Mx, E);             // lanes per slot of the line kernel = largest member tile
+        const int tps = dns_line_tps(d.lin ? Mz : Mx, E);   // lanes per slot of the line kernel = largest member tile
         p->line_tps = tps;
         int et = 1, lg = 0;
         while (et < tps && et < E) { et <<= 1; ++lg; }
@@ -192,7 +204,8 @@ int dns_plan_create(dns_plan** out, int Nx, int Ny, int Nz, int E, double Re, do
     p->ETf = pow2ceil(E) < 32 ? pow2ceil(E) : 32;
     { const int v = dns_option("etf"); if ((v == 4 || v == 8 || v == 16 || v == 32) && v <= pow2ceil(E)) p->ETf = v; }
     d.Kp = (((d.Ni + 1) / 2 + 7) / 8) * 8;
-    int ETy = pow2ceil(E) < 16 ? pow2ceil(E) : 16;
+    const int Etile = d.lin ? Eg : E;                    // a member tile of the per-pair kernel lies inside one kx group
+    int ETy = pow2ceil(Etile) < 16 ? pow2ceil(Etile) : 16;
     if (ETy < 4) ETy = 4;
     while (ETy > 4 && dns_ypair_smem(d.Ni, Ny, ETy) > 75 * 1024) ETy >>= 1;
     { const int v = dns_option("ety"); if (v == 4 || v == 8 || v == 16) ETy = v; }
@@ -220,6 +233,13 @@ int dns_plan_create(dns_plan** out, int Nx, int Ny, int Nz, int E, double Re, do
     return DNS_OK;
 }
 
+extern "C" {
+
+int dns_plan_create(dns_plan** out, int Nx, int Ny, int Nz, int E, double Re, double Lx, double Lz, double dt,
+                    int flow) {
+    return dns_create_common(out, Nx, Ny, Nz, E, Re, Lx, Lz, dt, flow, 0, nullptr, 0);
+}
+
 size_t dns_plan_workspace_bytes(const dns_plan* p) { return p ? p->workspace_bytes : 0; }
 
 int dns_plan_bind(dns_plan* p, void* ws, size_t bytes, void* stream) {
@@ -235,6 +255,7 @@ int dns_plan_bind(dns_plan* p, void* ws, size_t bytes, void* stream) {
     if (st != DNS_OK) { p->sticky = st; return st; }
     p->bound = true;
     p->has_state = false;
+    p->has_base = false;
     p->nstat = 0;
     return cuda_status(p, cudaMemsetAsync(ws, 0, p->workspace_bytes, p->stream));
 }
@@ -265,6 +286,7 @@ static cudaError_t stage_in(dns_plan* p, const double* vhat, const double* etaha
 
 int dns_set_state(dns_plan* p, const double* vhat, const double* etahat, const double* U00, const double* W00) {
     if (!p || !vhat || !etahat || !U00 || !W00) return DNS_EINVAL;
+    if (p->d.lin) return DNS_EINVAL;                      // a linearised-ensemble plan: use dns_lin_*
     if (p->sticky != DNS_OK) return p->sticky;
     if (!p->bound) return DNS_ESTATE;
     DnsDev& d = p->d;
@@ -292,6 +314,7 @@ int dns_set_state(dns_plan* p, const double* vhat, const double* etahat, const d
 
 int dns_add_increment(dns_plan* p, const double* dv, const double* deta) {
     if (!p || !dv || !deta) return DNS_EINVAL;
+    if (p->d.lin) return DNS_EINVAL;                      // a linearised-ensemble plan: use dns_lin_*
     if (p->sticky != DNS_OK) return p->sticky;
     if (!p->bound || !p->has_state) return DNS_ESTATE;
     DnsDev& d = p->d;
@@ -311,7 +334,7 @@ int dns_add_increment(dns_plan* p, const double* dv, const double* deta) {
 }
 
 int dns_plan_set_form(dns_plan* p, int form) {
-    if (!p || (form != DNS_FORM_CONVECTIVE && form != DNS_FORM_ROTATIONAL)) return DNS_EINVAL;
+    if (!p || p->d.lin || (form != DNS_FORM_CONVECTIVE && form != DNS_FORM_ROTATIONAL)) return DNS_EINVAL;
     if (p->has_state) return DNS_ESTATE;
     if (form != p->d.form) drop_step_graph(p);
     p->d.form = form;
@@ -319,7 +342,7 @@ int dns_plan_set_form(dns_plan* p, int form) {
 }
 
 int dns_plan_set_coupling(dns_plan* p, int mode, long long E_total) {
-    if (!p || (mode != DNS_COUPLING_NONE && mode != DNS_COUPLING_STREAMWISE_MEAN)) return DNS_EINVAL;
+    if (!p || p->d.lin || (mode != DNS_COUPLING_NONE && mode != DNS_COUPLING_STREAMWISE_MEAN)) return DNS_EINVAL;
     if (mode == DNS_COUPLING_STREAMWISE_MEAN && E_total < p->d.E) return DNS_EINVAL;
     if (p->has_state) return DNS_ESTATE;
     drop_step_graph(p);
@@ -338,6 +361,7 @@ int dns_plan_set_exchange(dns_plan* p, dns_exchange_fn fn, void* ctx) {
 
 int dns_step(dns_plan* p, int nsteps) {
     if (!p || nsteps < 0) return DNS_EINVAL;
+    if (p->d.lin) return DNS_EINVAL;                      // a linearised-ensemble plan: use dns_lin_*
     if (p->sticky != DNS_OK) return p->sticky;
     if (!p->bound || !p->has_state) return DNS_ESTATE;
     if (p->graph_state == 0 && nsteps > 0) build_step_graph(p);
@@ -355,6 +379,7 @@ int dns_step(dns_plan* p, int nsteps) {
 
 int dns_step_profile(dns_plan* p, int nsteps, double* ms) {
     if (!p || nsteps < 0 || !ms) return DNS_EINVAL;
+    if (p->d.lin) return DNS_EINVAL;                      // a linearised-ensemble plan: use dns_lin_*
     if (p->sticky != DNS_OK) return p->sticky;
     if (!p->bound || !p->has_state) return DNS_ESTATE;
     if (!p->ev_init) {
@@ -380,6 +405,7 @@ int dns_step_profile(dns_plan* p, int nsteps, double* ms) {
 
 int dns_get_state(dns_plan* p, double* vhat, double* etahat, double* U00, double* W00) {
     if (!p) return DNS_EINVAL;
+    if (p->d.lin) return DNS_EINVAL;                      // a linearised-ensemble plan: use dns_lin_*
     if (p->sticky != DNS_OK) return p->sticky;
     if (!p->bound || !p->has_state) return DNS_ESTATE;
     DnsDev& d = p->d;
@@ -407,6 +433,7 @@ int dns_get_state(dns_plan* p, double* vhat, double* etahat, double* U00, double
 
 int dns_diagnostics(dns_plan* p, double* out) {
     if (!p || !out) return DNS_EINVAL;
+    if (p->d.lin) return DNS_EINVAL;                      // a linearised-ensemble plan: use dns_lin_*
     if (p->sticky != DNS_OK) return p->sticky;
     if (!p->bound || !p->has_state) return DNS_ESTATE;
     DnsDev& d = p->d;
@@ -432,6 +459,7 @@ int dns_stats_reset(dns_plan* p) {
 
 int dns_stats_accumulate(dns_plan* p) {
     if (!p) return DNS_EINVAL;
+    if (p->d.lin) return DNS_EINVAL;                      // a linearised-ensemble plan: use dns_lin_*
     if (p->sticky != DNS_OK) return p->sticky;
     if (!p->bound || !p->has_state) return DNS_ESTATE;
     launch_stats(p);

@@ -16,6 +16,13 @@ struct DnsDev {
     int form;              // DNS_FORM_CONVECTIVE (u . grad u_i) or DNS_FORM_ROTATIONAL (omega x u, row f1)
     int coupling;          // DNS_COUPLING_NONE or DNS_COUPLING_STREAMWISE_MEAN (row f2)
     double invEtot;        // 1 / (members of the whole ensemble, over all ranks) for the coupled mean
+    // linearised forward / adjoint ensemble (row f3): every member has ONE streamwise mode, so the
+    // spectral arrays are [Ny][nkz][E] (nkx = 1, P = nkz) while the operator tables keep all nkxm = Nx/2 modes
+    int nkxm;              // streamwise modes in the kx and matrix tables (= nkx for a DNS plan)
+    int lin, Eg, nmodes;   // lin = 1: E = nmodes * Eg members, member e has streamwise mode nlist[e / Eg]
+    const int* nlist;      // [nmodes] (device)
+    double* base;          // [9][Ny][Mz] U V W Uy Vy Wy Uz Vz Wz of the frozen streamwise-mean base flow (physical z)
+    double* lin_scr;       // [E] energies, [E] gains, [Ny][E] partial sums
     int etl, ntl;          // mixed arrays are tile-major: member tile of 2^etl lanes, ntl = ceil(E / 2^etl) tiles
     double dt, Re, Uw, invMxMz;
     // plan-owned constant tables
@@ -74,6 +81,8 @@ struct dns_plan {
     cudaStream_t side = nullptr;               // the mean-flow kernel runs here, under the z-forward and per-pair kernels
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
     std::vector<void*> owned;                  // plan-owned device allocations
+    std::vector<int> nlist_host;               // linearised ensemble: streamwise mode of every kx group
+    bool has_base = false;
     void* workspace = nullptr;
     size_t workspace_bytes = 0;
     cudaStream_t stream = nullptr;
@@ -117,3 +126,12 @@ void launch_mean_out(dns_plan* p, double* U_abi, double* W_abi);
 void launch_normalise_state(dns_plan* p);
 void launch_diag(dns_plan* p, double t);
 void launch_stats(dns_plan* p);
+// linearised ensemble (kernels_lin.cu)
+void launch_diag_energy_part(dns_plan* p, double* part);      // part[Ny][E]: weighted per-plane energy sums
+void launch_lin_products(dns_plan* p, int adjoint);
+void launch_lin_normalise(dns_plan* p);
+void launch_lin_energy(dns_plan* p, double* out_dev);
+void launch_lin_gs(dns_plan* p);
+void launch_lin_base(dns_plan* lin, const dns_plan* dns, int member, cudaStream_t stream);
+int dns_create_common(dns_plan** out, int Nx, int Ny, int Nz, int E, double Re, double Lx, double Lz, double dt, int flow,
+                      int nmodes, const int* n_list, int Eg);

@@ -1,0 +1,190 @@
+// Linearised forward / adjoint ensemble (PAPER.md:296-317 and Appendix B, Eq. B.1-B.6 :390-417).
+// Every member is a disturbance with ONE streamwise wavenumber on a frozen streamwise-mean base flow (U, V, W)(y, z), so x is
+// analytic (d/dx = i kx) and only z is transformed.  A stage reuses the DNS kernels on arrays with a single kx row
+// (k_zinv* -> 8 mixed fields, k_zfwd*, k_ypair with the member's own single-kx matrices, "also valid for the adjoint
+// equations", :304); this file holds what is specific to the linear problem:
+//   k_lin_products : the linear vector that takes the place of u.grad u in Eq. 4-5, formed pointwise on the padded z grid
+//                    forward (B.2)  N_i = (U.grad) u_i + (u.grad) U_i
+//                    adjoint (B.5, reversed time, reading L1)  N_i = -(U.grad) lam_i - U_j d_i lam_j
+//   k_lin_base     : copies the kx = 0 column of one member of a DNS plan's mixed arrays = the base flow and its gradient
+//   k_lin_energy   : E_e = (1/2) sum_m sum_j w_j (|u|^2 + |v|^2 + |w|^2)                                  (B.1)
+//   k_lin_gs       : modified Gram-Schmidt in member order within each kx group, energy inner product     (:417)
+#include "dns_internal.h"
+
+namespace {
+
+__device__ __forceinline__ double2 cscale(double s, double2 a) { return make_double2(s * a.x, s * a.y); }
+__device__ __forceinline__ double2 cmuli(double s, double2 a) { return make_double2(-s * a.y, s * a.x); }      // (i s) a
+__device__ __forceinline__ double2 cadd3(double2 a, double2 b, double2 c) { return make_double2(a.x + b.x + c.x, a.y + b.y + c.y); }
+
+// grid = (ceil(E / 128), Mz, Ni); mixed arrays with one kx row are [Ny][Mz][Epad], Epad = ntl << etl
+__global__ void __launch_bounds__(128) k_lin_products(DnsDev d, int adjoint) {
+    const int e = blockIdx.x * blockDim.x + threadIdx.x, q = blockIdx.y, j = blockIdx.z + 1;
+    if (e >= d.E) return;
+    const size_t Epad = (size_t)d.ntl << d.etl, gi = ((size_t)j * d.Mz + q) * Epad + e, fs = d.Isz;
+    const size_t bi = (size_t)j * d.Mz + q, bs = (size_t)d.Ny * d.Mz;
+    const double kx = d.kx[d.nlist[e / d.Eg]];
+    const double U = d.base[bi], V = d.base[bs + bi], W = d.base[2 * bs + bi];
+    const double2 u = d.I8[gi], v = d.I8[fs + gi], w = d.I8[2 * fs + gi];
+    const double2 uy = d.I8[3 * fs + gi], wy = d.I8[4 * fs + gi];
+    const double2 uz = d.I8[5 * fs + gi], vz = d.I8[6 * fs + gi], wz = d.I8[7 * fs + gi];
+    const double2 ux = cmuli(kx, u), vx = cmuli(kx, v), wx = cmuli(kx, w);
+    const double2 vy = make_double2(-ux.x - wz.x, -ux.y - wz.y);      // continuity: dv/dy = -du/dx - dw/dz (interior rows)
+    // (U.grad) f for f = u, v, w
+    const double2 au = cadd3(cscale(U, ux), cscale(V, uy), cscale(W, uz));
+    const double2 av = cadd3(cscale(U, vx), cscale(V, vy), cscale(W, vz));
+    const double2 aw = cadd3(cscale(U, wx), cscale(V, wy), cscale(W, wz));
+    double2 Nu, Nv, Nw;
+    if (!adjoint) {
+        const double Uy = d.base[3 * bs + bi], Vy = d.base[4 * bs + bi], Wy = d.base[5 * bs + bi];
+        const double Uz = d.base[6 * bs + bi], Vz = d.base[7 * bs + bi], Wz = d.base[8 * bs + bi];
+        Nu = cadd3(au, cscale(Uy, v), cscale(Uz, w));                 // + (u.grad) U, dU/dx = 0
+        Nv = cadd3(av, cscale(Vy, v), cscale(Vz, w));
+        Nw = cadd3(aw, cscale(Wy, v), cscale(Wz, w));
+    } else {
+        const double2 bx = cadd3(cscale(U, ux), cscale(V, vx), cscale(W, wx));      // U_j d lam_j / dx
+        const double2 by = cadd3(cscale(U, uy), cscale(V, vy), cscale(W, wy));
+        const double2 bz = cadd3(cscale(U, uz), cscale(V, vz), cscale(W, wz));
+        Nu = make_double2(-au.x - bx.x, -au.y - bx.y);
+        Nv = make_double2(-av.x - by.x, -av.y - by.y);
+        Nw = make_double2(-aw.x - bz.x, -aw.y - bz.y);
+    }
+    d.I3[gi] = Nu;
+    d.I3[fs + gi] = Nv;
+    d.I3[2 * fs + gi] = Nw;
+}
+
+// base flow of the linear plan from the mixed arrays of a DNS plan (convective form: u v w Du Dw uz vz wz), kx = 0 column
+// of `member`, which is a real function of (y, z).  grid = (ceil(Mz / 64), Ni), block = 64
+__global__ void k_lin_base(DnsDev lin, DnsDev dns, int member) {
+    const int q = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y + 1;
+    if (q >= dns.Mz) return;
+    const size_t src = dns_mix_off(dns, j, q, 0, member), fs = dns.Isz;
+    const size_t bi = (size_t)j * lin.Mz + q, bs = (size_t)lin.Ny * lin.Mz;
+    const double U = dns.I8[src].x, V = dns.I8[fs + src].x, W = dns.I8[2 * fs + src].x;
+    const double Uy = dns.I8[3 * fs + src].x, Wy = dns.I8[4 * fs + src].x;
+    const double Uz = dns.I8[5 * fs + src].x, Vz = dns.I8[6 * fs + src].x, Wz = dns.I8[7 * fs + src].x;
+    lin.base[bi] = U; lin.base[bs + bi] = V; lin.base[2 * bs + bi] = W;
+    lin.base[3 * bs + bi] = Uy; lin.base[4 * bs + bi] = -Wz; lin.base[5 * bs + bi] = Wy;      // dV/dy = -dW/dz at kx = 0
+    lin.base[6 * bs + bi] = Uz; lin.base[7 * bs + bi] = Vz; lin.base[8 * bs + bi] = Wz;
+}
+
+// wall rows of the state are zero (Eq. 8); every (n, m) is a valid mode here (n >= 1)
+__global__ void k_lin_normalise(DnsDev d) {
+    const size_t row = (size_t)d.P * d.E;
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < row; i += (size_t)gridDim.x * blockDim.x) {
+        const double2 z = make_double2(0.0, 0.0);
+        d.vt[i] = z; d.et[i] = z;
+        d.vt[(size_t)(d.Ny - 1) * row + i] = z; d.et[(size_t)(d.Ny - 1) * row + i] = z;
+    }
+}
+
+// out[e] = sum_j part[j][e] in ascending j (part = the per-plane sums of k_diag_energy, already weighted)
+__global__ void k_lin_energy_rows(DnsDev d, const double* __restrict__ part, double* __restrict__ out) {
+    const int e = blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= d.E) return;
+    double s = 0.0;
+    for (int j = 0; j < d.Ny; ++j) s += part[(size_t)j * d.E + e];
+    out[e] = s;
+}
+
+// ---- modified Gram-Schmidt (reading L4): one CTA per kx group; the vectors are (v, eta) with their u, w (linear in the
+// state), the inner product is (1/2) sum_{m,j} w_j (conj(u_a) u_b + conj(v_a) v_b + conj(w_a) w_b).
+// Threads = EB member lanes x NSL element slots; partial sums are added in ascending slot order (deterministic).
+template <int EB> __global__ void __launch_bounds__(1024) k_lin_gs(DnsDev d) {
+    constexpr int NSL = 1024 / EB;
+    __shared__ double2 red[1024];
+    __shared__ double2 coef[EB];
+    const int g = blockIdx.x, bl = threadIdx.x % EB, slot = threadIdx.x / EB;
+    const int e_first = g * d.Eg, L = d.Ny * d.P;
+    double2* X[4] = {d.vt, d.et, d.uh, d.wh};
+    for (int a = 0; a < d.Eg; ++a) {
+        const int ea = e_first + a;
+        // norm of member a (all threads: lane 0 of every slot sums, the others idle)
+        double2 acc = make_double2(0.0, 0.0);
+        if (bl == 0)
+            for (int i = slot; i < L; i += NSL) {
+                const size_t gi = (size_t)i * d.E + ea;
+                const double2 u = d.uh[gi], v = d.vt[gi], w = d.wh[gi];
+                acc.x += d.w[i / d.P] * (u.x * u.x + u.y * u.y + v.x * v.x + v.y * v.y + w.x * w.x + w.y * w.y);
+            }
+        red[slot * EB + bl] = acc;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            double s = 0.0;
+            for (int k = 0; k < NSL; ++k) s += red[k * EB].x;
+            coef[0] = make_double2(1.0 / sqrt(0.5 * s), 0.0);
+        }
+        __syncthreads();
+        const double sc = coef[0].x;
+        for (int i = threadIdx.x; i < L; i += 1024) {
+            const size_t gi = (size_t)i * d.E + ea;
+#pragma unroll
+            for (int f = 0; f < 4; ++f) X[f][gi] = cscale(sc, X[f][gi]);
+        }
+        __syncthreads();
+        // projections of the later members of the group on member a, EB members at a time
+        for (int b0 = a + 1; b0 < d.Eg; b0 += EB) {
+            const int b = b0 + bl, eb = e_first + b;
+            acc = make_double2(0.0, 0.0);
+            if (b < d.Eg)
+                for (int i = slot; i < L; i += NSL) {
+                    const size_t ga = (size_t)i * d.E + ea, gb = (size_t)i * d.E + eb;
+                    const double wj = d.w[i / d.P];
+                    const double2 ua = d.uh[ga], va = d.vt[ga], wa = d.wh[ga], ub = d.uh[gb], vb = d.vt[gb], wb = d.wh[gb];
+                    // conj(a) * b
+                    acc.x += wj * (ua.x * ub.x + ua.y * ub.y + va.x * vb.x + va.y * vb.y + wa.x * wb.x + wa.y * wb.y);
+                    acc.y += wj * (ua.x * ub.y - ua.y * ub.x + va.x * vb.y - va.y * vb.x + wa.x * wb.y - wa.y * wb.x);
+                }
+            red[slot * EB + bl] = acc;
+            __syncthreads();
+            if (slot == 0) {
+                double2 s = make_double2(0.0, 0.0);
+                for (int k = 0; k < NSL; ++k) { s.x += red[k * EB + bl].x; s.y += red[k * EB + bl].y; }
+                coef[bl] = make_double2(0.5 * s.x, 0.5 * s.y);
+            }
+            __syncthreads();
+            if (b < d.Eg) {
+                const double2 c = coef[bl];
+                for (int i = slot; i < L; i += NSL) {
+                    const size_t ga = (size_t)i * d.E + ea, gb = (size_t)i * d.E + eb;
+#pragma unroll
+                    for (int f = 0; f < 4; ++f) {
+                        const double2 xa = X[f][ga];
+                        double2 xb = X[f][gb];
+                        xb.x -= c.x * xa.x - c.y * xa.y;
+                        xb.y -= c.x * xa.y + c.y * xa.x;
+                        X[f][gb] = xb;
+                    }
+                }
+            }
+            __syncthreads();
+        }
+    }
+}
+
+}  // namespace
+
+void launch_lin_products(dns_plan* p, int adjoint) {
+    const DnsDev& d = p->d;
+    dim3 grid((d.E + 127) / 128, d.Mz, d.Ni);
+    k_lin_products<<<grid, 128, 0, p->stream>>>(d, adjoint);
+}
+void launch_lin_base(dns_plan* lin, const dns_plan* dns, int member, cudaStream_t stream) {
+    dim3 grid((dns->d.Mz + 63) / 64, dns->d.Ni);
+    k_lin_base<<<grid, 64, 0, stream>>>(lin->d, dns->d, member);
+}
+void launch_lin_normalise(dns_plan* p) { k_lin_normalise<<<148, 256, 0, p->stream>>>(p->d); }
+void launch_lin_energy(dns_plan* p, double* out_dev) {
+    const DnsDev& d = p->d;
+    double* part = d.lin_scr + 2 * (size_t)d.E;
+    launch_diag_energy_part(p, part);
+    k_lin_energy_rows<<<(d.E + 127) / 128, 128, 0, p->stream>>>(d, part, out_dev);
+}
+void launch_lin_gs(dns_plan* p) {
+    const DnsDev& d = p->d;
+    if (d.Eg <= 4) k_lin_gs<4><<<d.nmodes, 1024, 0, p->stream>>>(d);
+    else if (d.Eg <= 8) k_lin_gs<8><<<d.nmodes, 1024, 0, p->stream>>>(d);
+    else if (d.Eg <= 16) k_lin_gs<16><<<d.nmodes, 1024, 0, p->stream>>>(d);
+    else k_lin_gs<32><<<d.nmodes, 1024, 0, p->stream>>>(d);
+}

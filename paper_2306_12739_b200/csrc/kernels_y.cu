@@ -249,15 +249,30 @@ k_ypair(DnsDev d, const __grid_constant__ CUtensorMap tmN, const __grid_constant
     constexpr int NWN = NWNT, NC = 8 * NT * NWN, ET = NC >> 1, ld = NC + 4;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
     const int mt = warp % KS2, wn = warp / KS2;
-    const int ntile_e = (d.E + ET - 1) / ET;
-    const int p = 1 + bid / ntile_e, e0 = (bid % ntile_e) * ET;
-    const int n = p / d.nkz, mi = p % d.nkz;
+    // DNS plan: pair p = (n, mi) != (0, 0), member tiles over all E.  Linearised ensemble (row f3): the arrays hold one
+    // streamwise mode per member, p = mi, and a member tile lies inside one kx group (members g Eg .. (g+1) Eg - 1 share n)
+    int p, e0, eend, n, mi;
+    if (d.lin) {
+        const int ntile_g = (d.Eg + ET - 1) / ET, ntile_e = d.nmodes * ntile_g, tile = bid % ntile_e, g = tile / ntile_g;
+        p = bid / ntile_e;
+        e0 = g * d.Eg + (tile % ntile_g) * ET;
+        eend = (g + 1) * d.Eg;
+        n = d.nlist[g];
+        mi = p;
+    } else {
+        const int ntile_e = (d.E + ET - 1) / ET;
+        p = 1 + bid / ntile_e;
+        e0 = (bid % ntile_e) * ET;
+        eend = d.E;
+        n = p / d.nkz;
+        mi = p % d.nkz;
+    }
     const int mabs = mi < d.nzh ? mi : d.nkz - mi;
     const double kx = d.kx[n], kz = d.kz[mi], alpha = kx * kx + kz * kz, ialpha = 1.0 / alpha;
     const int hi = stage == 0 ? 0 : 1;
     const double hdt = (stage == 0 ? 0.5 : 1.0) * d.dt;
     const size_t BB = (size_t)Kp * Kp;
-    const double* mA = d.matsP + (((size_t)hi * d.nkx * d.nzh + (size_t)n * d.nzh + mabs) * 6) * BB;
+    const double* mA = d.matsP + (((size_t)hi * d.nkxm * d.nzh + (size_t)n * d.nzh + mabs) * 6) * BB;
     const double* Dsd = d.Dfrag;            // dd -> s
     const double* Dds = d.Dfrag + BB;       // s -> dd
     const size_t PS = ((size_t)Ni * ld + 15) & ~(size_t)15;      // panel pitch: a multiple of 128 B (TMA destination)
@@ -274,7 +289,7 @@ k_ypair(DnsDev d, const __grid_constant__ CUtensorMap tmN, const __grid_constant
 
     // ---- stage the inputs: one TMA tile per field (box = Ni rows x ld doubles, landing in the padded panel layout;
     //      the 4 pad columns of every row are the first two members of the neighbouring tile: never used)
-    const int nvalid = d.E - e0 < ET ? d.E - e0 : ET;
+    const int nvalid = eend - e0 < ET ? eend - e0 : ET;
     if (threadIdx.x == 0) {
         mbar_init(&bar, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -298,7 +313,7 @@ k_ypair(DnsDev d, const __grid_constant__ CUtensorMap tmN, const __grid_constant
     const bool sok = i < Kh, dok = i < Kho;
     const int col0 = 8 * NT * wn;
     const int offS = (sok ? i : 0) * ld + col0 + 2 * t, offD = (dok ? Ji : 0) * ld + col0 + 2 * t;
-    auto eokf = [&](int nt) { return (e0 + (col0 >> 1) + 4 * nt + t) < d.E; };
+    auto eokf = [&](int nt) { return (e0 + (col0 >> 1) + 4 * nt + t) < eend; };
     const size_t gS = pbase + (size_t)(i + 1) * rowstride + (col0 >> 1) + t;      // + 4 nt : natural row i
     const size_t gD = pbase + (size_t)(Ji + 1) * rowstride + (col0 >> 1) + t;     // natural row J i
 
@@ -647,7 +662,7 @@ __global__ void __launch_bounds__(256) k_diag_energy(DnsDev d, double* __restric
         double s[1];
         plane_mode_sums<1>(d, j, 0, sm, [&](int p, size_t gi, double* a) {
             const double2 u = d.uh[gi], v = d.vt[gi], w = d.wh[gi];
-            const double cn = (p / d.nkz) == 0 ? 1.0 : 2.0;
+            const double cn = (!d.lin && (p / d.nkz) == 0) ? 1.0 : 2.0;     // a stored mode with kx > 0 stands for +-kx
             a[0] += cn * (u.x * u.x + u.y * u.y + v.x * v.x + v.y * v.y + w.x * w.x + w.y * w.y);
         }, s, e0, EB);
         const int e = e0 + threadIdx.x;
@@ -772,7 +787,8 @@ int dns_ypair_encode_maps(dns_plan* p) {
 template <int NT, int NWN> static void ypair_launch(dns_plan* p, int stage, int derive_only) {
     const DnsDev& d = p->d;
     const int KS2 = d.Kp >> 3, ET = 4 * NT * NWN;
-    const unsigned grid = (unsigned)((d.P - 1) * ((d.E + ET - 1) / ET));
+    const unsigned grid = d.lin ? (unsigned)(d.nkz * d.nmodes * ((d.Eg + ET - 1) / ET))
+                                : (unsigned)((d.P - 1) * ((d.E + ET - 1) / ET));
     const size_t smem = dns_ypair_smem(d.Ni, d.Ny, ET);
 #define LAUNCH(K)                                                                                     \
     {                                                                                                 \
@@ -839,6 +855,7 @@ void launch_ens(dns_plan* p, int phase) {
     const int nwarps = 3 * d.Ni * d.nkz + d.Ni * d.Mz;
     k_ens<<<(nwarps + 7) / 8, 256, 0, p->stream>>>(d, phase);
 }
+void launch_diag_energy_part(dns_plan* p, double* part) { k_diag_energy<<<p->d.Ny, 256, 0, p->stream>>>(p->d, part); }
 void launch_diag(dns_plan* p, double t) {
     const DnsDev& d = p->d;
     double* part = d.diag + (size_t)d.E * 6;

@@ -201,9 +201,9 @@ int dns_host_precompute(dns_plan* p) {
         for (int j = 1; j < N; ++j) w[j] = (double)(2.0L * v[j] / N);
     }
     // ---- wavenumbers and FFT twiddles
-    std::vector<double> kx(d.nkx), kz(d.nkz);
+    std::vector<double> kx(d.nkxm), kz(d.nkz);
     const real LX = p->Lx, LZ = p->Lz;
-    for (int n = 0; n < d.nkx; ++n) kx[n] = (double)(2.0L * PI_L * n / LX);
+    for (int n = 0; n < d.nkxm; ++n) kx[n] = (double)(2.0L * PI_L * n / LX);
     for (int i = 0; i < d.nkz; ++i) {
         int m = (i < d.nzh) ? i : i - d.nkz;     // 0..Nz/2-1, -(Nz/2-1)..-1
         kz[i] = (double)(2.0L * PI_L * m / LZ);
@@ -220,7 +220,7 @@ int dns_host_precompute(dns_plan* p) {
         return t;
     };
     // ---- per-(alpha, h) inverses (Listing 1 + Listing 3, Eq. 12-13)
-    const int nA = d.nkx * d.nzh;
+    const int nA = d.nkxm * d.nzh;
     const size_t NN = (size_t)Ni * Ni;
     const int Kp = d.Kp, Kh = (Ni + 1) / 2, Kho = Ni / 2;
     const size_t BB = (size_t)Kp * Kp;
@@ -315,6 +315,7 @@ int dns_host_precompute(dns_plan* p) {
     d.Ugam = upload(p, Ugam, &err);
     d.twx = upload(p, twiddles(d.Mx), &err);
     d.twz = upload(p, twiddles(d.Mz), &err);
+    if (d.lin) d.nlist = upload(p, p->nlist_host, &err);
     if (err == cudaErrorMemoryAllocation) return DNS_ENOMEM;
     return err == cudaSuccess ? DNS_OK : DNS_ECUDA;
 }
