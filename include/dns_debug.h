@@ -34,6 +34,7 @@ int dns_debug_stage(dns_plan* plan, int stage);
  *   "line_ring" input ring of the line kernel with 16-lane tiles: 0 half an item deep, 1 a whole item (8 | 6 fields)
  *   "line_pair" Mx = 54, 72 (12 slots, 6 busy in the first pass), convective form: 0 one transform per round, 1 two per
  *              round with two exchange buffers, 4 two per round with four exchange buffers (default)
+ *   "pdl"      1: programmatic dependent launch between the stage kernels (measured slower: off by default)
  *   "line_alt" 1: Mx = 72 as 8 x 9 on 9 one-warp slots in the line kernel instead of 6 x 12 on 12 slots (measured slower)
  * Errors: DNS_EINVAL (unknown name). */
 int dns_debug_set_option(const char* name, int value);

@@ -103,6 +103,33 @@ struct dns_plan {
     bool ev_init = false;
 };
 
+int dns_option(const char* name);            // test / tuning options (include/dns_debug.h); -1 = default
+// Programmatic dependent launch between the kernels of a stage (option "pdl" = 1; OFF by default): every stage kernel lets
+// its successor start launching at once (DNS_PDL_TRIGGER at its top) and waits for its predecessor to complete and flush
+// (DNS_PDL_WAIT) before it touches anything a kernel wrote; every CTA of every such kernel executes the wait, so completion
+// stays transitive along the chain.  Measured slower on every configuration (config 1: 59.4 -> 66.4 us per step, config 4:
+// 12.02 -> 12.62 ms): the early CTAs of the successor take shared memory and registers from the running kernel, and the
+// small configurations are bound by the latency of one CTA's dependent chain, not by launch gaps.  Without the launch
+// attribute both instructions are no-ops.
+#if defined(__CUDACC__)
+#define DNS_PDL_TRIGGER() asm volatile("griddepcontrol.launch_dependents;" ::: "memory")
+#define DNS_PDL_WAIT() asm volatile("griddepcontrol.wait;" ::: "memory")
+template <class... KArgs, class... Args>
+inline cudaError_t dns_launch(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = dns_option("pdl") == 1 ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
+}
+#endif
+
 // host precompute (plan.cu)
 int dns_host_precompute(dns_plan* p);
 bool dns_factor_len(int M, int* R1, int* R2);
@@ -112,7 +139,6 @@ int dns_line_tps(int Mx, int E);
 void launch_zinv(dns_plan* p, const double2* vin, const double2* ein);
 void launch_ens(dns_plan* p, int phase);     // phase 0: sums -> d.ens ; 1: d.ens / Etot -> members ; 2: both
 size_t dns_ens_count(const DnsDev& d);       // doubles in d.ens
-int dns_option(const char* name);            // test / tuning options (include/dns_debug.h); -1 = default
 void launch_line(dns_plan* p);
 void launch_zfwd(dns_plan* p);
 void launch_ypair(dns_plan* p, int stage, int derive_only);

@@ -41,6 +41,8 @@ __device__ __forceinline__ const double2* zinv_src(const DnsDev& d, int f, const
 #endif
 template <int R1, int R2>
 __global__ void __launch_bounds__(256, DNS_FFT_MINB) k_zinv(DnsDev d, const double2* __restrict__ vin, const double2* __restrict__ ein, int etlog, int NB) {
+    DNS_PDL_TRIGGER();
+    DNS_PDL_WAIT();
     constexpr int M = R1 * R2;
     extern __shared__ double2 sm[];
     const int ET = 1 << etlog, e_l = threadIdx.x & (ET - 1), slot = threadIdx.x >> etlog, nslots = blockDim.x >> etlog;
@@ -108,6 +110,8 @@ __global__ void __launch_bounds__(256, DNS_FFT_MINB) k_zinv(DnsDev d, const doub
 // grid.x = Ni * nblk_n * ntile_e, grid.y = 3 fields; block = 256
 template <int R1, int R2>
 __global__ void __launch_bounds__(256) k_zfwd(DnsDev d, int etlog, int NB) {
+    DNS_PDL_TRIGGER();
+    DNS_PDL_WAIT();
     constexpr int M = R1 * R2;
     extern __shared__ double2 sm[];
     const int ET = 1 << etlog, e_l = threadIdx.x & (ET - 1), slot = threadIdx.x >> etlog, nslots = blockDim.x >> etlog;
@@ -164,6 +168,8 @@ __global__ void __launch_bounds__(256) k_zfwd(DnsDev d, int etlog, int NB) {
 //   forward (decimation in frequency): thread h holds x(i + H h); a_h(i) = (x(i) +- x(i+H)) w^(h i); X(2m + h) = DFT_H(a_h)(m)
 template <int H, bool TP>
 __global__ void __launch_bounds__(128) k_zinv_r(DnsDev d, const double2* __restrict__ vin, const double2* __restrict__ ein) {
+    DNS_PDL_TRIGGER();
+    DNS_PDL_WAIT();
     constexpr int M = 2 * H, LO = H / 3, HI = 2 * H / 3;   // positions 2i+h < M/3 <=> i < LO ; > 2M/3 <=> i > HI (i == HI: h = 1 only)
     static_assert(H % 3 == 0, "padded length must be 3/2 of an even grid");
     const int h = threadIdx.x & 1;
@@ -224,6 +230,8 @@ __global__ void __launch_bounds__(128) k_zinv_r(DnsDev d, const double2* __restr
 
 template <int H>
 __global__ void __launch_bounds__(128) k_zfwd_r(DnsDev d) {
+    DNS_PDL_TRIGGER();
+    DNS_PDL_WAIT();
     constexpr int M = 2 * H, LO = H / 3, HI = 2 * H / 3;
     const int h = threadIdx.x & 1;
     const int nper = d.nkx * d.E, nblk = (nper + 63) >> 6;
@@ -275,6 +283,8 @@ __device__ __forceinline__ double2 quad_dft4(double2 z, int l1, int l0) {
 
 template <int H, bool TP>
 __global__ void __launch_bounds__(128) k_zinv_r4(DnsDev d, const double2* __restrict__ vin, const double2* __restrict__ ein) {
+    DNS_PDL_TRIGGER();
+    DNS_PDL_WAIT();
     constexpr int M = 4 * H, LO = H / 3, HI = 2 * H / 3;   // positions 4i+r < M/3 <=> i < LO ; > 2M/3 <=> i > HI (i == HI: r >= 1)
     static_assert(H % 3 == 0, "padded length must be 3/2 of an even grid");
     const int l0 = threadIdx.x & 1, l1 = (threadIdx.x >> 1) & 1, r = 2 * l1 + l0, qo = l1 + 2 * l0;
@@ -329,6 +339,8 @@ __global__ void __launch_bounds__(128) k_zinv_r4(DnsDev d, const double2* __rest
 
 template <int H>
 __global__ void __launch_bounds__(128) k_zfwd_r4(DnsDev d) {
+    DNS_PDL_TRIGGER();
+    DNS_PDL_WAIT();
     constexpr int M = 4 * H, LO = H / 3, HI = 2 * H / 3;
     const int l0 = threadIdx.x & 1, l1 = (threadIdx.x >> 1) & 1, qi = 2 * l1 + l0, r = l1 + 2 * l0;
     const int nper = d.nkx * d.E, nblk = (nper + 31) >> 5;
@@ -358,24 +370,24 @@ __global__ void __launch_bounds__(128) k_zfwd_r4(DnsDev d) {
 template <int H> void zinv_r4_launch(dns_plan* p, const double2* vin, const double2* ein) {
     const DnsDev& d = p->d;
     dim3 grid((unsigned)(d.Ni * ((d.nkx * d.E + 31) / 32)), d.form == DNS_FORM_ROTATIONAL ? 6 : 8);
-    k_zinv_r4<H, false><<<grid, 128, 0, p->stream>>>(d, vin, ein);
+    dns_launch(k_zinv_r4<H, false>, grid, dim3(128), 0, p->stream, d, vin, ein);
 }
 template <int H> void zfwd_r4_launch(dns_plan* p) {
     const DnsDev& d = p->d;
     dim3 grid((unsigned)(d.Ni * ((d.nkx * d.E + 31) / 32)), 3);
-    k_zfwd_r4<H><<<grid, 128, 0, p->stream>>>(d);
+    dns_launch(k_zfwd_r4<H>, grid, dim3(128), 0, p->stream, d);
 }
 
 template <int H> void zinv_r_launch(dns_plan* p, const double2* vin, const double2* ein) {
     const DnsDev& d = p->d;
     constexpr bool TP = H <= 24;                      // measured: helps Mz <= 48, costs occupancy above
     dim3 grid((unsigned)(d.Ni * ((d.nkx * d.E + 63) / 64)), d.form == DNS_FORM_ROTATIONAL ? 6 : (TP ? 5 : 8));
-    k_zinv_r<H, TP><<<grid, 128, 0, p->stream>>>(d, vin, ein);
+    dns_launch(k_zinv_r<H, TP>, grid, dim3(128), 0, p->stream, d, vin, ein);
 }
 template <int H> void zfwd_r_launch(dns_plan* p) {
     const DnsDev& d = p->d;
     dim3 grid((unsigned)(d.Ni * ((d.nkx * d.E + 63) / 64)), 3);
-    k_zfwd_r<H><<<grid, 128, 0, p->stream>>>(d);
+    dns_launch(k_zfwd_r<H>, grid, dim3(128), 0, p->stream, d);
 }
 bool use_zreg(int Mz) {
     return dns_option("zreg") != 0 && (Mz == 24 || Mz == 36 || Mz == 48 || Mz == 72 || Mz == 96);
@@ -401,7 +413,7 @@ template <int R1, int R2> void zinv_launch(dns_plan* p, const double2* vin, cons
     static size_t have = 0;
     ensure_smem(kern, smem, &have);
     dim3 grid((unsigned)(d.Ni * ((d.nkx + NB - 1) / NB) * ((d.E + ET - 1) / ET)), d.form == DNS_FORM_ROTATIONAL ? 6 : 5);
-    kern<<<grid, 256, smem, p->stream>>>(d, vin, ein, etlog, NB);
+    dns_launch(kern, grid, dim3(256), smem, p->stream, d, vin, ein, etlog, NB);
 }
 
 template <int R1, int R2> void zfwd_launch(dns_plan* p) {
@@ -416,7 +428,7 @@ template <int R1, int R2> void zfwd_launch(dns_plan* p) {
     static size_t have = 0;
     ensure_smem(kern, smem, &have);
     dim3 grid((unsigned)(d.Ni * ((d.nkx + NB - 1) / NB) * ((d.E + ET - 1) / ET)), 3);
-    kern<<<grid, 256, smem, p->stream>>>(d, etlog, NB);
+    dns_launch(kern, grid, dim3(256), smem, p->stream, d, etlog, NB);
 }
 
 }  // namespace

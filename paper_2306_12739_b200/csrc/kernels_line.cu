@@ -130,6 +130,7 @@ __global__ void __launch_bounds__(SL * TPS * NG, MINB) k_line(DnsDev d, int nite
     constexpr int BUF = (R1 * PI > R2 * PF) ? R1 * PI : R2 * PF;
     constexpr int SLOT = NKX * TPS;                          // double2 per ring slot
     static_assert(NST == NSEQ || 2 * NST == NSEQ || SIX8, "ring depth");
+    DNS_PDL_TRIGGER();
     extern __shared__ __align__(128) unsigned char smraw[];
     const LineSmem L = line_smem(R1, R2, SL, TPS, NG, NST, NBUF);
     double* kxs = reinterpret_cast<double*>(smraw + L.kxs);
@@ -154,6 +155,7 @@ __global__ void __launch_bounds__(SL * TPS * NG, MINB) k_line(DnsDev d, int nite
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     }
     __syncthreads();
+    DNS_PDL_WAIT();                                          // the mixed fields of k_zinv are complete from here on
 
     const size_t fstride = d.Isz;
     const int E = d.E;
@@ -467,7 +469,7 @@ template <int R1, int R2, int SL, int TPS, int NG, int NST8, int MINB, bool ROT,
     }
     int grid = (nitems + NG - 1) / NG;
     if (grid > p->line_grid) grid = p->line_grid;
-    kern<<<grid, SL * TPS * NG, L.total, p->stream>>>(d, nitems);
+    dns_launch(kern, dim3(grid), dim3(SL * TPS * NG), (size_t)L.total, p->stream, d, nitems);
 }
 template <int R1, int R2, int SL, int TPS, int NG, int NST8, int MINB, bool ROT, bool PAIR, int NBUF> void line_launch_form(dns_plan* p) {
     // full member tiles (ET = TPS): always with 16 lanes (chosen for E >= 16 only), with 8 lanes when E >= 8

@@ -69,15 +69,29 @@ __device__ __forceinline__ void gemm2(double (&accS)[NT][2], double (&accD)[NT][
     const double2* AfD = reinterpret_cast<const double2*>(AD) + (size_t)mt * KS2 * 32 + lane;
     const double* BcS = BS + col0 + g;
     const double* BcD = BD + col0 + g;
+    // Specialised sweep lengths (KS2T != 0: Kp = 16, 24, 32, 48) always have Kp <= Ni, so no row index ever needs the
+    // clamp below: the row pointers are then one per-thread base plus compile-time multiples of ld (immediate offsets).
+    const double* SF = BcS + t * ld;
+    const double* SR = BcS + (Ni - 1 - t) * ld;
+    const double* DF = BcD + t * ld;
+    const double* DR = BcD + (Ni - 1 - t) * ld;
 #pragma unroll
     for (int ks2 = 0; ks2 < KS2; ++ks2) {
         const double2 aS = __ldg(AfS + ks2 * 32), aD = __ldg(AfD + ks2 * 32);
-        const int k = 8 * ks2 + t;
-        const int f0 = min(k, Ni - 1), f1 = min(k + 4, Ni - 1), r0 = max(Ni - 1 - k, 0), r1 = max(Ni - 5 - k, 0);
-        const double* s0 = BcS + (REVS ? r0 : f0) * ld;
-        const double* s1 = BcS + (REVS ? r1 : f1) * ld;
-        const double* d0 = BcD + (REVD ? r0 : f0) * ld;
-        const double* d1 = BcD + (REVD ? r1 : f1) * ld;
+        const double *s0, *s1, *d0, *d1;
+        if constexpr (KS2T != 0) {
+            s0 = REVS ? SR - (8 * ks2) * ld : SF + (8 * ks2) * ld;
+            s1 = REVS ? SR - (8 * ks2 + 4) * ld : SF + (8 * ks2 + 4) * ld;
+            d0 = REVD ? DR - (8 * ks2) * ld : DF + (8 * ks2) * ld;
+            d1 = REVD ? DR - (8 * ks2 + 4) * ld : DF + (8 * ks2 + 4) * ld;
+        } else {
+            const int k = 8 * ks2 + t;
+            const int f0 = min(k, Ni - 1), f1 = min(k + 4, Ni - 1), r0 = max(Ni - 1 - k, 0), r1 = max(Ni - 5 - k, 0);
+            s0 = BcS + (REVS ? r0 : f0) * ld;
+            s1 = BcS + (REVS ? r1 : f1) * ld;
+            d0 = BcD + (REVD ? r0 : f0) * ld;
+            d1 = BcD + (REVD ? r1 : f1) * ld;
+        }
 #pragma unroll
         for (int nt = 0; nt < NT; ++nt) { dmma(accS[nt], aS.x, s0[8 * nt]); dmma(accD[nt], aD.x, d0[8 * nt]); }
 #pragma unroll
@@ -242,6 +256,7 @@ template <int NT, int NWNT, int KS2T>
 __global__ void __launch_bounds__(KS2T ? 32 * KS2T * NWNT : 1024, ypair_minb(32 * KS2T * NWNT))
 k_ypair(DnsDev d, const __grid_constant__ CUtensorMap tmN, const __grid_constant__ CUtensorMap tmV,
         const __grid_constant__ CUtensorMap tmE, int stage, int derive_only) {
+    DNS_PDL_TRIGGER();
     extern __shared__ __align__(128) double smy[];
     __shared__ uint64_t bar;
     const int bid = blockIdx.x;
@@ -290,6 +305,7 @@ k_ypair(DnsDev d, const __grid_constant__ CUtensorMap tmN, const __grid_constant
     // ---- stage the inputs: one TMA tile per field (box = Ni rows x ld doubles, landing in the padded panel layout;
     //      the 4 pad columns of every row are the first two members of the neighbouring tile: never used)
     const int nvalid = eend - e0 < ET ? eend - e0 : ET;
+    DNS_PDL_WAIT();                                          // the index arithmetic above overlaps the z-forward kernel's tail
     if (threadIdx.x == 0) {
         mbar_init(&bar, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -550,6 +566,8 @@ k_ypair(DnsDev d, const __grid_constant__ CUtensorMap tmN, const __grid_constant
 // per-pair kernels: it needs only the plane sums written by the line kernel
 __global__ void __launch_bounds__(256) k_mean(DnsDev d, int stage, int derive_only) {
     extern __shared__ __align__(128) double smm[];
+    DNS_PDL_TRIGGER();
+    DNS_PDL_WAIT();
     mean_body(d, stage, derive_only, blockIdx.x, smm);
 }
 
@@ -800,7 +818,7 @@ template <int NT, int NWN> static void ypair_launch(dns_plan* p, int stage, int 
             attr_smem = smem;                                                                         \
         }                                                                                             \
         const CUtensorMap* tm = reinterpret_cast<const CUtensorMap*>(p->tmaps);                       \
-        kern<<<grid, 32 * KS2 * NWN, smem, p->stream>>>(d, tm[0], tm[1], tm[2], stage, derive_only); \
+        dns_launch(kern, dim3(grid), dim3(32 * KS2 * NWN), smem, p->stream, d, tm[0], tm[1], tm[2], stage, derive_only); \
     }
     switch (KS2) {
         case 2: LAUNCH(2) break;
