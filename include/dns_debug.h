@@ -32,8 +32,9 @@ int dns_debug_stage(dns_plan* plan, int stage);
  *   "ety","nty" member tile (4, 8, 16) and n-tiles per warp (1, 2, 4) of the per-pair kernel
  *   "line_tps" lanes per slot of the line kernel (4, 8, 16)
  *   "line_ring" input ring of the line kernel with 16-lane tiles: 0 half an item deep, 1 a whole item (8 | 6 fields)
- *   "line_pair" Mx = 54, 72 (12 slots, 6 busy in the first pass), convective form: 0 one transform per round, 1 two per
- *              round with two exchange buffers, 4 two per round with four exchange buffers (default)
+ *   "line_pair" Mx = 54, 72 (12 slots, 6 busy in the first pass): 0 one transform per round; 1 two per round with two
+ *              exchange buffers, 5 with four buffers and a half ring (both convective form only); default: two per round,
+ *              four buffers, 6-slot ring
  *   "pdl"      1: programmatic dependent launch between the stage kernels (measured slower: off by default)
  *   "line_alt" 1: Mx = 72 as 8 x 9 on 9 one-warp slots in the line kernel instead of 6 x 12 on 12 slots (measured slower)
  * Errors: DNS_EINVAL (unknown name). */

@@ -510,15 +510,16 @@ template <int R1, int R2, int SL> static void line_launch_tps(dns_plan* p) {
                 const int ring = dns_option("line_ring");
                 const bool whole = !big && (ring < 0 ? p->d.form == DNS_FORM_ROTATIONAL : ring == 1);
                 constexpr int MB = SL == 8 ? 3 : 2;
-                // paired rounds where half of the slots would idle in the first pass (SL = 2 R1: Mx = 54, 72), convective
-                // form (config 4: 1732 -> 1565 us with two exchange buffers, 1519 us with four; the rotational form has
-                // three transforms and gains nothing).  Option "line_pair": 0 off, 1 two buffers, 4 four buffers (default)
+                // paired rounds where half of the slots would idle in the first pass (SL = 2 R1: Mx = 54, 72).  Config 4,
+                // convective: 1732 us one transform per round, 1565 us paired with two exchange buffers, 1519 us with four and a
+                // half ring, 1452 us with four and the 6-slot ring (default); rotational: 1063 -> 998 us (whole ring, four
+                // buffers).  Option "line_pair": 0 off, 1 two buffers (convective), 5 four buffers + half ring (convective)
                 if constexpr (SL == 2 * R1 && !big) {
                     const int pair = dns_option("line_pair");
                     const bool rotf = p->d.form == DNS_FORM_ROTATIONAL;
                     if (pair == 1 && !rotf) { line_launch<R1, R2, SL, 16, 1, 4, MB, true>(p); break; }
                     if (pair == 5 && !rotf) { line_launch<R1, R2, SL, 16, 1, 4, MB, true, 4>(p); break; }
-                    if (pair != 0 && !rotf) { line_launch<R1, R2, SL, 16, 1, 6, MB, true, 4>(p); break; }
+                    if (pair != 0) { line_launch<R1, R2, SL, 16, 1, 6, MB, true, 4>(p); break; }
                 }
                 if constexpr (!big) {
                     if (whole) { line_launch<R1, R2, SL, 16, 1, 8, MB>(p); break; }
