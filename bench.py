@@ -267,21 +267,27 @@ def main():
                              "GBps": c["bytes"] / per_launch_s * 1e-9, "TFLOPs": c["flops"] / per_launch_s * 1e-12,
                              "alg_bytes_per_launch": c["bytes"], "alg_flops_per_launch": c["flops"],
                              "bound": "hbm" if t_hbm >= t_alu else "fp64",
-                             "frac": max(t_hbm, t_alu) / per_launch_s}
+                             "frac": max(t_hbm, t_alu) / per_launch_s,
+                             "traffic": traffic_lookup(name, cfg, rot)[0]}
         return plan, value, ms_max, clocks, kernels
+
+    def traffic_lookup(kernel, cfg, rot):
+        """DRAM bytes per launch of one kernel class from the committed ncu capture of the same workload and form
+        (profiles/dominant_kernel_traffic.json, written from `ncu --set full` reports; see profiles/r2f_kernels.md)."""
+        tpath = os.path.join(ROOT, "profiles", "dominant_kernel_traffic.json")
+        try:
+            for rec in json.load(open(tpath)):
+                if rec.get("kernel") == kernel and rec.get("workload") == cfg.name and \
+                        rec.get("form", "convective") == ("rotational" if rot else "convective"):
+                    return rec.get("dram_bytes_per_launch"), rec.get("source")
+        except Exception:
+            pass
+        return None, None
 
     def roofline_of(kernels, cfg, rot):
         dom = max(kernels, key=lambda k: kernels[k]["share"])
         kd = kernels[dom]
-        traffic, tsrc = None, None
-        tpath = os.path.join(ROOT, "profiles", "dominant_kernel_traffic.json")
-        try:
-            for rec in json.load(open(tpath)):
-                if rec.get("kernel") == dom and rec.get("workload") == cfg.name and \
-                        rec.get("form", "convective") == ("rotational" if rot else "convective"):
-                    traffic, tsrc = rec.get("dram_bytes_per_launch"), rec.get("source")
-        except Exception:
-            pass
+        traffic, tsrc = traffic_lookup(dom, cfg, rot)
         if kd["bound"] == "hbm":
             r = {"bound": "hbm", "achieved": kd["GBps"], "peak": hbm_peak, "unit": "GB/s", "frac": kd["GBps"] / hbm_peak}
         else:
