@@ -228,8 +228,11 @@ __global__ void __launch_bounds__(128) k_zinv_r(DnsDev d, const double2* __restr
     }
 }
 
+// H = 36 (Mz = 72): two CTAs per SM fit with any register count, so the allocator is left free (254 instead of its own
+// 178 registers: every load of the line stays in flight; config 4: 477 -> 371 us per launch).  Shorter lines keep the
+// allocator's choice (0 = unspecified): more registers would cost them a CTA per SM (measured slower for H = 24).
 template <int H>
-__global__ void __launch_bounds__(128) k_zfwd_r(DnsDev d) {
+__global__ void __launch_bounds__(128, H == 36 ? 1 : 0) k_zfwd_r(DnsDev d) {
     DNS_PDL_TRIGGER();
     DNS_PDL_WAIT();
     constexpr int M = 2 * H, LO = H / 3, HI = 2 * H / 3;
