@@ -273,7 +273,7 @@ def main():
 
     def traffic_lookup(kernel, cfg, rot):
         """DRAM bytes per launch of one kernel class from the committed ncu capture of the same workload and form
-        (profiles/dominant_kernel_traffic.json, written from `ncu --set full` reports; see profiles/r2f_kernels.md)."""
+        (profiles/dominant_kernel_traffic.json, written from `ncu --set full` reports; see profiles/r2g_kernels.md)."""
         tpath = os.path.join(ROOT, "profiles", "dominant_kernel_traffic.json")
         try:
             for rec in json.load(open(tpath)):

@@ -217,3 +217,36 @@ def test_shared_memory_z_kernels_both_forms():
             assert_errs(errs, 1, TOL_1)
     finally:
         binding.dns_debug_set_option("zreg", -1)
+
+
+@pytest.mark.parametrize("Nx", [36, 48])
+def test_line_kernel_round_variants(Nx):
+    """Mx = 54 and 72 in the 16-lane family (ragged second member tile): the default line kernel runs two transforms per
+    round with four exchange buffers (6-slot ring in the convective form); options "line_pair" = 0 / 1 / 5 select one
+    transform per round, two exchange buffers, four buffers with a half ring; "pdl" = 1 adds programmatic dependent launch.
+    Every variant against the oracle, and all variants bit-identical to each other (same arithmetic per line)."""
+    cfg = inputs.Config(1, inputs.COUETTE, 350.0, 1.9 * PI, 1.1 * PI, Nx, 13, 16, 17, 0.01, 1, 0.1, 0, box=3)
+    st = inputs.make_state(cfg)
+    idx = [0, 8, 15, 16]
+    for form in (0, ROT):
+        o = Oracle(*inputs.plan_args(cfg, E=len(idx)), form=form)
+        o.set_state(st["vhat"][idx], st["etahat"][idx], st["U00"][idx], st["W00"][idx])
+        o.step(2)
+        ref = None
+        for name, val in (("line_pair", -1), ("line_pair", 0), ("line_pair", 1), ("line_pair", 5), ("pdl", 1)):
+            assert binding.dns_debug_set_option(name, val) == binding.DNS_OK
+            try:
+                plan = binding.Plan(*inputs.plan_args(cfg), form=form)
+                plan.set_state(st["vhat"], st["etahat"], st["U00"], st["W00"])
+                plan.step(2)
+                got = plan.get_state()
+                plan.close()
+            finally:
+                binding.dns_debug_set_option(name, -1)
+            assert field_err(got[0][idx], o.v) < TOL_1 * 10 and field_err(got[1][idx], o.eta) < TOL_1 * 10, (name, val, form)
+            assert field_err(got[2][idx], o.U) < TOL_1 * 10
+            if ref is None:
+                ref = got
+            else:
+                for a, b in zip(ref, got):
+                    assert np.array_equal(a, b), (name, val, form)
