@@ -564,7 +564,7 @@ k_ypair(DnsDev d, const __grid_constant__ CUtensorMap tmN, const __grid_constant
 
 // mean flow as its own small launch (8 members per CTA); api.cu runs it on a side stream under the z-forward and
 // per-pair kernels: it needs only the plane sums written by the line kernel
-__global__ void __launch_bounds__(256) k_mean(DnsDev d, int stage, int derive_only) {
+__global__ void __launch_bounds__(512) k_mean(DnsDev d, int stage, int derive_only) {
     extern __shared__ __align__(128) double smm[];
     DNS_PDL_TRIGGER();
     DNS_PDL_WAIT();
@@ -845,7 +845,10 @@ void launch_mean(dns_plan* p, int stage, int derive_only, cudaStream_t stream) {
     const size_t smem = (size_t)6 * d.Ny * 8 * sizeof(double);
     static size_t attr_smem = 48 * 1024;
     if (smem > attr_smem) { cudaFuncSetAttribute(k_mean, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr_smem = smem; }   // Ny >= 129
-    k_mean<<<(d.E + 7) / 8, 256, smem, stream>>>(d, stage, derive_only);
+    // small ensembles: the kernel is one or a few CTAs whose serial rounds over the rows ARE its duration (and, below about
+    // 16 members, longer than the z-forward + per-pair kernels it runs beside): 64 row slots finish Ny <= 66 in one round
+    const int threads = (d.E <= 8 && d.Ni > 32) ? 512 : 256;
+    k_mean<<<(d.E + 7) / 8, threads, smem, stream>>>(d, stage, derive_only);
 }
 
 void launch_abi_to_internal(dns_plan* p, const double2* src, double2* dst, int accumulate) {
