@@ -273,13 +273,14 @@ def main():
 
     def traffic_lookup(kernel, cfg, rot):
         """DRAM bytes per launch of one kernel class from the committed ncu capture of the same workload and form
-        (profiles/dominant_kernel_traffic.json, written from `ncu --set full` reports; see profiles/r2g_kernels.md)."""
-        tpath = os.path.join(ROOT, "profiles", "dominant_kernel_traffic.json")
+        (profiles/dominant_kernel_traffic.csv, copied from `ncu --set full` reports; see profiles/r2g_kernels.md)."""
+        tpath = os.path.join(ROOT, "profiles", "dominant_kernel_traffic.csv")
         try:
-            for rec in json.load(open(tpath)):
+            import csv
+            for rec in csv.DictReader(open(tpath)):
                 if rec.get("kernel") == kernel and rec.get("workload") == cfg.name and \
                         rec.get("form", "convective") == ("rotational" if rot else "convective"):
-                    return rec.get("dram_bytes_per_launch"), rec.get("source")
+                    return float(rec["dram_bytes_per_launch"]), rec.get("source")
         except Exception:
             pass
         return None, None
