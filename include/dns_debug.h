@@ -35,6 +35,8 @@ int dns_debug_stage(dns_plan* plan, int stage);
  *   "line_pair" Mx = 54, 72 (12 slots, 6 busy in the first pass): 0 one transform per round; 1 two per round with two
  *              exchange buffers, 5 with four buffers and a half ring (both convective form only); default: two per round,
  *              four buffers, 6-slot ring
+ *   "zinv_tp"  0: convective form without the L2 prefetch of the two-pass z inverse (Mz <= 48) and, for Mz = 72, with the
+ *              one-pass kernel (8 output fields) instead of the two-pass one
  *   "pdl"      1: programmatic dependent launch between the stage kernels (measured slower: off by default)
  *   "line_alt" 1: Mx = 72 as 8 x 9 on 9 one-warp slots in the line kernel instead of 6 x 12 on 12 slots (measured slower)
  * Errors: DNS_EINVAL (unknown name). */

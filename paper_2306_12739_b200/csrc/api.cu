@@ -13,7 +13,7 @@ namespace {
 
 // test / tuning options of include/dns_debug.h (process-wide; -1 = default)
 struct Option { const char* name; int value; };
-Option g_options[] = {{"graph", -1}, {"zreg", -1}, {"etf", -1}, {"ety", -1}, {"nty", -1}, {"line_tps", -1}, {"line_alt", -1}, {"line_ring", -1}, {"line_pair", -1}, {"pdl", -1}};
+Option g_options[] = {{"graph", -1}, {"zreg", -1}, {"etf", -1}, {"ety", -1}, {"nty", -1}, {"line_tps", -1}, {"line_alt", -1}, {"line_ring", -1}, {"line_pair", -1}, {"pdl", -1}, {"zinv_tp", -1}};
 
 size_t align256(size_t b) { return (b + 255) & ~(size_t)255; }
 

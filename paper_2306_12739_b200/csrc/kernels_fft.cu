@@ -167,7 +167,7 @@ __global__ void __launch_bounds__(256) k_zfwd(DnsDev d, int etlog, int NB) {
 //                                  x(k + H h) = E(k) +- w^k O(k), w = exp(-2 pi i / M) on swapped data (swap identity)
 //   forward (decimation in frequency): thread h holds x(i + H h); a_h(i) = (x(i) +- x(i+H)) w^(h i); X(2m + h) = DFT_H(a_h)(m)
 template <int H, bool TP>
-__global__ void __launch_bounds__(128) k_zinv_r(DnsDev d, const double2* __restrict__ vin, const double2* __restrict__ ein) {
+__global__ void __launch_bounds__(128) k_zinv_r(DnsDev d, const double2* __restrict__ vin, const double2* __restrict__ ein, int pf) {
     DNS_PDL_TRIGGER();
     DNS_PDL_WAIT();
     constexpr int M = 2 * H, LO = H / 3, HI = 2 * H / 3;   // positions 2i+h < M/3 <=> i < LO ; > 2M/3 <=> i > HI (i == HI: h = 1 only)
@@ -200,6 +200,26 @@ __global__ void __launch_bounds__(128) k_zinv_r(DnsDev d, const double2* __restr
             if (ok && (i != HI || h == 1)) {
                 a[i] = ldg2(src + (size_t)mi * d.E);
                 if (deriv) kzv[i] = __ldg(d.kz + mi);
+            }
+        }
+    }
+    if (TP && pass == 0 && pf > 0) {
+        // two-pass CTAs issue no loads during their second transform: keep the DRAM queue fed with the lines of the CTA
+        // that will replace this one (pf blocks ahead in launch order), as L2 prefetches
+        const unsigned bn = blockIdx.x + (unsigned)pf;
+        if (bn < gridDim.x) {
+            const int jn = bn / nblk + 1, qn = (bn % nblk) * 64 + (threadIdx.x >> 1);
+            if (qn < nper) {
+                const int nn = qn / d.E, en = qn - nn * d.E;
+                const double2* sn = zinv_src(d, f, vin, ein) + ((size_t)jn * d.nkx + nn) * d.nkz * d.E + en;
+                if ((en & 7) == 0) {                           // one prefetch per 128-byte line (8 members)
+#pragma unroll
+                    for (int i = 0; i < H; ++i)
+                        if (i < LO || i >= HI) {
+                            const int mi = i < LO ? 2 * i + h : 2 * i + h - M / 3 - 1;
+                            if (i != HI || h == 1) asm volatile("prefetch.global.L2 [%0];" ::"l"(sn + (size_t)mi * d.E));
+                        }
+                }
             }
         }
     }
@@ -383,9 +403,21 @@ template <int H> void zfwd_r4_launch(dns_plan* p) {
 
 template <int H> void zinv_r_launch(dns_plan* p, const double2* vin, const double2* ein) {
     const DnsDev& d = p->d;
-    constexpr bool TP = H <= 24;                      // measured: helps Mz <= 48, costs occupancy above
-    dim3 grid((unsigned)(d.Ni * ((d.nkx * d.E + 63) / 64)), d.form == DNS_FORM_ROTATIONAL ? 6 : (TP ? 5 : 8));
-    dns_launch(k_zinv_r<H, TP>, grid, dim3(128), 0, p->stream, d, vin, ein);
+    const bool rot = d.form == DNS_FORM_ROTATIONAL;
+    const unsigned nb = (unsigned)(d.Ni * ((d.nkx * d.E + 63) / 64));
+    // Two passes (u, v, w also give their z-derivative from the same inputs: 3 S less DRAM traffic): always for Mz <= 48.
+    // Mz = 72: alone it gains little (a thread in its second transform issues no loads and the DRAM queue runs shallow:
+    // 985 -> 948 us on config 4), with the L2 prefetch of the lines of a CTA half a wave ahead it gives 915 us (flat for
+    // distances of 74 .. 296 CTAs).  Option "zinv_tp" = 0: the one-pass kernel with 8 output fields.
+    if constexpr (H == 36) {
+        if (!rot && dns_option("zinv_tp") != 0) {
+            dns_launch(k_zinv_r<H, true>, dim3(nb, 5), dim3(128), 0, p->stream, d, vin, ein, 148);
+            return;
+        }
+    }
+    constexpr bool TP = H <= 24;
+    dim3 grid(nb, rot ? 6 : (TP ? 5 : 8));
+    dns_launch(k_zinv_r<H, TP>, grid, dim3(128), 0, p->stream, d, vin, ein, (TP && !rot && dns_option("zinv_tp") != 0) ? 148 : 0);   // Mz = 48: 75.6 -> 73.2 us on config 2
 }
 template <int H> void zfwd_r_launch(dns_plan* p) {
     const DnsDev& d = p->d;

@@ -219,13 +219,15 @@ def test_shared_memory_z_kernels_both_forms():
         binding.dns_debug_set_option("zreg", -1)
 
 
-@pytest.mark.parametrize("Nx", [36, 48])
-def test_line_kernel_round_variants(Nx):
+@pytest.mark.parametrize("Nx,Nz", [(36, 16), (48, 16), (16, 48)])
+def test_line_kernel_round_variants(Nx, Nz):
     """Mx = 54 and 72 in the 16-lane family (ragged second member tile): the default line kernel runs two transforms per
     round with four exchange buffers (6-slot ring in the convective form); options "line_pair" = 0 / 1 / 5 select one
-    transform per round, two exchange buffers, four buffers with a half ring; "pdl" = 1 adds programmatic dependent launch.
+    transform per round, two exchange buffers, four buffers with a half ring; "pdl" = 1 adds programmatic dependent launch;
+    "zinv_tp" = 0 takes the L2 prefetch out of the two-pass z inverse and, for Mz = 72 (third case), selects the one-pass
+    z inverse instead of the two-pass one.
     Every variant against the oracle, and all variants bit-identical to each other (same arithmetic per line)."""
-    cfg = inputs.Config(1, inputs.COUETTE, 350.0, 1.9 * PI, 1.1 * PI, Nx, 13, 16, 17, 0.01, 1, 0.1, 0, box=3)
+    cfg = inputs.Config(1, inputs.COUETTE, 350.0, 1.9 * PI, 1.1 * PI, Nx, 13, Nz, 17, 0.01, 1, 0.1, 0, box=3)
     st = inputs.make_state(cfg)
     idx = [0, 8, 15, 16]
     for form in (0, ROT):
@@ -233,7 +235,7 @@ def test_line_kernel_round_variants(Nx):
         o.set_state(st["vhat"][idx], st["etahat"][idx], st["U00"][idx], st["W00"][idx])
         o.step(2)
         ref = None
-        for name, val in (("line_pair", -1), ("line_pair", 0), ("line_pair", 1), ("line_pair", 5), ("pdl", 1)):
+        for name, val in (("line_pair", -1), ("line_pair", 0), ("line_pair", 1), ("line_pair", 5), ("pdl", 1), ("zinv_tp", 0)):
             assert binding.dns_debug_set_option(name, val) == binding.DNS_OK
             try:
                 plan = binding.Plan(*inputs.plan_args(cfg), form=form)
