@@ -196,6 +196,8 @@ def main():
     ap.add_argument("--members", type=int, default=0, help="override E per GPU (config 5 sweep)")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true",
+                    help="skip the threaded end-to-end measurement (for runs under ncu only: `e2e` is then null)")
     ap.add_argument("--sweep", action="store_true",
                     help="BASELINE config 5: one JSON line per ensemble size E in inputs.SWEEP_E (per-kernel times and "
                          "roofline fractions versus E); not the default bench line")
@@ -273,7 +275,7 @@ def main():
 
     def traffic_lookup(kernel, cfg, rot):
         """DRAM bytes per launch of one kernel class from the committed ncu capture of the same workload and form
-        (profiles/dominant_kernel_traffic.csv, copied from `ncu --set full` reports; see profiles/r2g_kernels.md)."""
+        (profiles/dominant_kernel_traffic.csv, copied from `ncu --set full` reports; see profiles/r2k_kernels.md)."""
         tpath = os.path.join(ROOT, "profiles", "dominant_kernel_traffic.csv")
         try:
             import csv
@@ -359,7 +361,7 @@ def main():
                             ws=plan.workspace_bytes, roofline=roofline_of(kernels, cfg, rot))
             plan.close()
         head = res[forms[0]]
-        e2e = measure_e2e(cfg, cfg_all, st, 1 if (args.sweep or cfg.E < 8) else 4)
+        e2e = None if args.no_e2e else measure_e2e(cfg, cfg_all, st, 1 if (args.sweep or cfg.E < 8) else 4)
 
         line = {
             "metric": METRIC, "value": head["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
