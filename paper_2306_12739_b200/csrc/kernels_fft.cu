@@ -305,7 +305,7 @@ __device__ __forceinline__ double2 quad_dft4(double2 z, int l1, int l0) {
 }
 
 template <int H, bool TP>
-__global__ void __launch_bounds__(128) k_zinv_r4(DnsDev d, const double2* __restrict__ vin, const double2* __restrict__ ein, int pf) {
+__global__ void __launch_bounds__(128) k_zinv_r4(DnsDev d, const double2* __restrict__ vin, const double2* __restrict__ ein) {
     DNS_PDL_TRIGGER();
     DNS_PDL_WAIT();
     constexpr int M = 4 * H, LO = H / 3, HI = 2 * H / 3;   // positions 4i+r < M/3 <=> i < LO ; > 2M/3 <=> i > HI (i == HI: r >= 1)
@@ -337,24 +337,6 @@ __global__ void __launch_bounds__(128) k_zinv_r4(DnsDev d, const double2* __rest
             if (ok && (i != HI || r >= 1)) {
                 a[i] = ldg2(src + (size_t)mi * d.E);
                 if (deriv) kzv[i] = __ldg(d.kz + mi);
-            }
-        }
-    }
-    if (TP && pass == 0 && pf > 0) {                          // see k_zinv_r: keep the DRAM queue fed during the second transform
-        const unsigned bn = blockIdx.x + (unsigned)pf;
-        if (bn < gridDim.x) {
-            const int jn = bn / nblk + 1, qn = (bn % nblk) * 32 + (threadIdx.x >> 2);
-            if (qn < nper) {
-                const int nn = qn / d.E, en = qn - nn * d.E;
-                const double2* sn = zinv_src(d, f, vin, ein) + ((size_t)jn * d.nkx + nn) * d.nkz * d.E + en;
-                if ((en & 7) == 0) {
-#pragma unroll
-                    for (int i = 0; i < H; ++i)
-                        if (i < LO || i >= HI) {
-                            const int mi = i < LO ? 4 * i + r : 4 * i + r - M / 3 - 1;
-                            if (i != HI || r >= 1) asm volatile("prefetch.global.L2 [%0];" ::"l"(sn + (size_t)mi * d.E));
-                        }
-                }
             }
         }
     }
@@ -408,15 +390,11 @@ __global__ void __launch_bounds__(128) k_zfwd_r4(DnsDev d) {
     }
 }
 
+// Mz = 96: one pass per output field (the two-pass variant with the L2 prefetch of k_zinv_r measured no better: 198 against 195 us)
 template <int H> void zinv_r4_launch(dns_plan* p, const double2* vin, const double2* ein) {
     const DnsDev& d = p->d;
-    const bool rot = d.form == DNS_FORM_ROTATIONAL;
-    const unsigned nb = (unsigned)(d.Ni * ((d.nkx * d.E + 31) / 32));
-    if (!rot && dns_option("zinv_tp") == 3) {            // EXPERIMENT: two passes + prefetch for Mz = 96
-        dns_launch(k_zinv_r4<H, true>, dim3(nb, 5), dim3(128), 0, p->stream, d, vin, ein, 148);
-        return;
-    }
-    dns_launch(k_zinv_r4<H, false>, dim3(nb, rot ? 6 : 8), dim3(128), 0, p->stream, d, vin, ein, 0);
+    dim3 grid((unsigned)(d.Ni * ((d.nkx * d.E + 31) / 32)), d.form == DNS_FORM_ROTATIONAL ? 6 : 8);
+    dns_launch(k_zinv_r4<H, false>, grid, dim3(128), 0, p->stream, d, vin, ein);
 }
 template <int H> void zfwd_r4_launch(dns_plan* p) {
     const DnsDev& d = p->d;
