@@ -273,6 +273,8 @@ def main():
                              "traffic": traffic_lookup(name, cfg, rot)[0]}
         return plan, value, ms_max, clocks, kernels
 
+    ncu_extra = {}
+
     def traffic_lookup(kernel, cfg, rot):
         """DRAM bytes per launch of one kernel class from the committed ncu capture of the same workload and form
         (profiles/dominant_kernel_traffic.csv, copied from `ncu --set full` reports; see profiles/r2k_kernels.md)."""
@@ -282,6 +284,7 @@ def main():
             for rec in csv.DictReader(open(tpath)):
                 if rec.get("kernel") == kernel and rec.get("workload") == cfg.name and \
                         rec.get("form", "convective") == ("rotational" if rot else "convective"):
+                    ncu_extra[(kernel, rot)] = float(rec.get("fp64_pipe_active_pct") or 0.0)
                     return float(rec["dram_bytes_per_launch"]), rec.get("source")
         except Exception:
             pass
@@ -296,6 +299,9 @@ def main():
         else:
             r = {"bound": "tensor" if dom == "ypair_dmma" else "alu", "achieved": kd["TFLOPs"], "peak": fp64_peak,
                  "unit": "TFLOP/s", "frac": kd["TFLOPs"] / fp64_peak}
+        # context from the same ncu capture: how busy the fp64 pipe was (the line kernel is bound by fp64 instruction issue,
+        # DESIGN.md sections 5 and 7; DFMA and DMMA share that pipe)
+        r["fp64_pipe_active_pct_ncu"] = ncu_extra.get((dom, rot))
         r.update({"traffic": traffic, "traffic_source": tsrc, "kernel": dom, "peak_source": peak_src + "; " + fp64_src,
                   "alg_bytes_per_launch": kd["alg_bytes_per_launch"], "us_per_launch": kd["us_per_launch"],
                   "share_of_step": kd["share"]})
