@@ -222,12 +222,12 @@ def main():
     base = inputs.CONFIGS[5 if args.sweep else args.config]
     sizes = list(inputs.SWEEP_E) if args.sweep else [args.members or base.E]
     hbm_peak, peak_src = measured_peaks()
-    fp64 = {"dfma_tflops": None, "dmma_tflops": None}
-    for kind, key in ((0, "dfma_tflops"), (1, "dmma_tflops")):
+    fp64 = {"dfma_tflops": None, "dmma_tflops": None, "mixed_dfma_dmma_tflops": None}
+    for kind, key in ((0, "dfma_tflops"), (1, "dmma_tflops"), (2, "mixed_dfma_dmma_tflops")):
         st_, tf = binding.dns_debug_fp64_peak(kind, 0.4)
         if st_ == binding.DNS_OK:
             fp64[key] = tf
-    fp64_peak = max([v for v in fp64.values() if v] or [FP64_PEAK_FALLBACK])
+    fp64_peak = max([v for k, v in fp64.items() if v and k != "mixed_dfma_dmma_tflops"] or [FP64_PEAK_FALLBACK])
     fp64_src = ("fp64 %.1f TFLOP/s measured live (dns_debug_fp64_peak: DFMA %.1f, DMMA.8x8x4 %.1f; 0.4 s each)"
                 % (fp64_peak, fp64["dfma_tflops"] or 0.0, fp64["dmma_tflops"] or 0.0)) if fp64["dfma_tflops"] \
         else "fp64 %.1f TFLOP/s fallback (units x clock)" % FP64_PEAK_FALLBACK

@@ -43,7 +43,8 @@ int dns_debug_stage(dns_plan* plan, int stage);
 int dns_debug_set_option(const char* name, int value);
 
 /* dns_debug_fp64_peak -- measures the sustained fp64 throughput of the current device with a register-resident
- * microbenchmark (no memory traffic): kind 0 = DFMA chains, kind 1 = DMMA.8x8x4 (mma.sync m8n8k4 f64) chains, run back
+ * microbenchmark (no memory traffic): kind 0 = DFMA chains, kind 1 = DMMA.8x8x4 (mma.sync m8n8k4 f64) chains, kind 2 = both kinds
+ * interleaved in every thread (8 DFMA + 2 DMMA chains: the sum stays below either peak, i.e. the two share one pipe), run back
  * to back for about `seconds` of device time; *tflops receives 2 x fused multiply-adds per second / 1e12.  This is the
  * denominator of every fp64 roofline fraction bench.py prints ("measure sustained fp64 ... exactly as
  * MEASURED_PEAKS.json did for bf16").  Errors: DNS_EINVAL, DNS_ECUDA. */

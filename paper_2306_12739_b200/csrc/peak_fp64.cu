@@ -44,10 +44,39 @@ __global__ void __launch_bounds__(256) k_peak_dmma(double* out, double a, double
     if (s == 12345.678) out[0] = s;
 }
 
+// kind 2: every thread interleaves CHAINS independent DFMA chains with MIXM independent DMMA chains.  If the two instruction
+// kinds had pipes of their own the sum of their rates would exceed either peak; on B200 it does not.
+constexpr int MIXM = 2;
+__global__ void __launch_bounds__(256) k_peak_mix(double* out, double a, double b) {
+    double x[CHAINS];
+    double acc[MIXM][2];
+#pragma unroll
+    for (int c = 0; c < CHAINS; ++c) x[c] = (double)(threadIdx.x + c);
+#pragma unroll
+    for (int c = 0; c < MIXM; ++c) acc[c][0] = acc[c][1] = (double)(threadIdx.x + c);
+#pragma unroll 1
+    for (int it = 0; it < ITERS; ++it) {
+#pragma unroll
+        for (int c = 0; c < CHAINS; ++c) {
+            x[c] = fma(x[c], a, b);
+            if (c < MIXM)
+                asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                             : "+d"(acc[c][0]), "+d"(acc[c][1])
+                             : "d"(a), "d"(b));
+        }
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int c = 0; c < CHAINS; ++c) s += x[c];
+#pragma unroll
+    for (int c = 0; c < MIXM; ++c) s += acc[c][0] + acc[c][1];
+    if (s == 12345.678) out[0] = s;
+}
+
 }  // namespace
 
 extern "C" int dns_debug_fp64_peak(int kind, double seconds, double* tflops) {
-    if (!tflops || (kind != 0 && kind != 1) || !(seconds > 0.0) || seconds > 30.0) return DNS_EINVAL;
+    if (!tflops || kind < 0 || kind > 2 || !(seconds > 0.0) || seconds > 30.0) return DNS_EINVAL;
     int dev = 0, nsm = 0;
     if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
         cudaGetLastError();
@@ -62,11 +91,12 @@ extern "C" int dns_debug_fp64_peak(int kind, double seconds, double* tflops) {
     }
     const int grid = nsm * 8, block = 256;
     // fused multiply-adds per launch: DFMA = 1 per thread and instruction; DMMA m8n8k4 = 8*8*4 = 256 per warp and instruction
-    const double fma_per_launch = kind == 0 ? (double)grid * block * CHAINS * ITERS
-                                            : (double)grid * (block / 32) * CHAINS * ITERS * 256.0;
+    const double fma_dfma = (double)grid * block * CHAINS * ITERS, fma_dmma = (double)grid * (block / 32) * ITERS * 256.0;
+    const double fma_per_launch = kind == 0 ? fma_dfma : (kind == 1 ? fma_dmma * CHAINS : fma_dfma + fma_dmma * MIXM);
     auto launch = [&]() {
         if (kind == 0) k_peak_dfma<<<grid, block>>>(out, 0.999999, 1e-9);
-        else k_peak_dmma<<<grid, block>>>(out, 0.999999, 1e-9);
+        else if (kind == 1) k_peak_dmma<<<grid, block>>>(out, 0.999999, 1e-9);
+        else k_peak_mix<<<grid, block>>>(out, 0.999999, 1e-9);
     };
     for (int w = 0; w < 3; ++w) launch();
     cudaDeviceSynchronize();
