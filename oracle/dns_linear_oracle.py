@@ -30,7 +30,11 @@ the modified (sequential) variant in member order within a kx group.
 Pins (tests/test_oracle_pins_linear.py): P19a the forward linear vector is the exact central difference of the pinned
 nonlinear oracle about the base flow; P19b the discrete adjoint identity <lam, N_fwd(u)> = <N_adj(lam), u> on resolved
 states; P19c the power iteration against the generalised eigenvalues (final vs initial energy Gram matrices) of the forward
-oracle on a basis of smooth clamped profiles; P19d Gram-Schmidt orthonormality; P19e Orr-Sommerfeld growth on a laminar base flow.  Parity with the author's MATLAB output: UNPINNED.
+oracle on a basis of smooth clamped profiles; P19d Gram-Schmidt orthonormality; P19e Orr-Sommerfeld growth on a laminar base
+flow; P19f the RK3 stage weights that step() re-states and the direction of time of the adjoint leg,
+against Kutta's amplification polynomial 1 + z + z^2/2 + z^3/6 in the inviscid limit, forward (z) and adjoint (-z); P19g the
+1/(2V) of inner() (B.1) against the pinned Oracle.energy of a DNS state holding the same single-kx disturbance.
+Parity with the author's MATLAB output: UNPINNED.
 """
 from __future__ import annotations
 

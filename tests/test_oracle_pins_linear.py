@@ -8,7 +8,11 @@ f3; PAPER.md:296-317 and Appendix B :390-417), against what the mathematics fixe
         forward propagator (energy norm), first and second optimal;
   P19d  Gram-Schmidt leaves an energy-orthonormal set and only normalises the first vector of every kx group;
   P19e  on a laminar base flow a forward step amplifies an Orr-Sommerfeld eigenmode by exp(lambda dt) (independent
-        eigen-solve of test_oracle_pins.py), with a time-step factor t_f = 5 as in :315.
+        eigen-solve of test_oracle_pins.py), with a time-step factor t_f = 5 as in :315;
+  P19f  the stage weights of LinearEnsemble.step and the reversed time of the adjoint leg (:411-417):
+        one inviscid step multiplies a Squire mode by Kutta's polynomial in z (forward) and in -z (adjoint); three wrong
+        weightings are kept red;
+  P19g  the 1/(2V) of LinearEnsemble.inner (Eq. B.1, :396) against the pinned Oracle.energy of the same disturbance.
 All tests run on CPU (`-m "not gpu"`).
 """
 import numpy as np
@@ -169,3 +173,107 @@ def test_P19e_laminar_base_flow_orr_sommerfeld_growth_with_time_step_factor():
     fac = np.vdot(vi, L.v[0, mi]) / np.vdot(vi, vi)
     expect = np.exp(lam[k] * nsteps * dt_lin)
     assert abs(fac - expect) < 2e-5 * abs(expect), (fac, expect)
+
+
+# ------------------------------------------------------------------------------------------------ P19f / P19g
+def _lin_inviscid_squire_step(adjoint, dt=0.15, Ny=25, n=2, step=None):
+    """One step of the LINEAR oracle on a Squire mode (v = 0, kz = 0, eta = 1e-9 g(y)) over the parabola U = 1 - y^2 at
+    Re = 1e12 (Crank-Nicolson part switched off).  Eq. 17-18 give u = 0, w = i eta / kx, so the forward vector of B.2 is
+    N_w = i kx U w and Eq. 5 gives G = i kx U eta: every collocation point obeys d eta_j/dt = -i kx U(y_j) eta_j.  In B.5
+    (v = 0, kz = 0: U_i grad lam_i vanishes with u) the reversed-time equation is d eta_j/d tau = +i kx U(y_j) eta_j.
+    Returns (eta_0, eta_1, z_j) with z_j = -i kx U(y_j) dt, the FORWARD exponent."""
+    Lx = 2 * PI
+    L = LinearEnsemble(12, Ny, 12, [n], 1, 1e12, Lx, PI, dt, POISEUILLE_CMF)
+    if step is not None:
+        L.step = step.__get__(L)
+    y = L.o.y
+    z0 = np.zeros((11, Ny), complex)
+    L.set_base(z0, z0, 1 - y ** 2, np.zeros(Ny))
+    eh = np.zeros((1, 11, Ny), complex)
+    eh[0, 0] = 1e-9 * (1 - y ** 2) * (1 + 0.3 * y) * np.exp(0.7j * y)
+    L.set_state(np.zeros_like(eh), eh)
+    e0 = L.eta[0, 0].copy()
+    L.step(1, adjoint)
+    assert np.abs(L.v).max() < 1e-16
+    return e0, L.eta[0, 0].copy(), -1j * (2 * PI * n / Lx) * (1 - y ** 2) * dt
+
+
+def _mutated_lin_step(mutation):
+    """LinearEnsemble.step with one wrong stage weighting (the three the round-2 review found invisible to P19a-e)."""
+    def step(self, nsteps=1, adjoint=False):
+        for _ in range(int(nsteps)):
+            v_t, e_t = self.v, self.eta
+            F0, G0 = self._forcing_all(adjoint)
+            self.v, self.eta = self._stage(v_t, e_t, 0.5, F0, G0)
+            F1, G1 = self._forcing_all(adjoint)
+            c2 = (F1, G1) if mutation == "stage2_F1" else (2.0 * F1 - F0, 2.0 * G1 - G0)
+            self.v, self.eta = self._stage(v_t, e_t, 1.0, *c2)
+            F2, G2 = self._forcing_all(adjoint)
+            if mutation == "stage3_quarter":
+                c3 = ((F0 + 2.0 * F1 + F2) / 4.0, (G0 + 2.0 * G1 + G2) / 4.0)
+            elif mutation == "stage3_F1":
+                c3 = (F1, G1)
+            else:
+                c3 = ((F0 + 4.0 * F1 + F2) / 6.0, (G0 + 4.0 * G1 + G2) / 6.0)
+            self.v, self.eta = self._stage(v_t, e_t, 1.0, *c3)
+    return step
+
+
+@pytest.mark.parametrize("adjoint", [False, True])
+def test_P19f_rk3_weights_of_the_linear_step_kutta_polynomial(adjoint):
+    """LinearEnsemble.step re-states the stage weights of PAPER.md:120-126 (F^0 with h = 1/2; 2 F^1 - F^0; (F^0 + 4 F^1 +
+    F^2)/6) and does not call the pinned Oracle.step, so it gets the pin P16 gives that one: one inviscid step multiplies
+    eta(y_j) by EXACTLY Kutta's polynomial 1 + z + z^2/2 + z^3/6 -- with z = -i kx U(y_j) dt forward (B.2) and with -z for
+    the adjoint, which runs in reversed time (B.5, reading L1; "evolved backwards").  kx dt = 0.3 makes the
+    cubic term 4.5e-3 against a tolerance of 1e-10 (measured on the oracle: 1e-12).  The sign of the exponent also pins the
+    direction of time of the adjoint leg, which P19b (an identity at one instant) cannot see.  Red on: stage 2 <- F^1,
+    stage 3 <- (F^0 + 2 F^1 + F^2)/4, stage 3 <- F^1 (test_P19f_detects_wrong_rk3_weights), all of which passed P19a-e."""
+    e0, e1, z = _lin_inviscid_squire_step(adjoint)
+    if adjoint:
+        z = -z
+    kutta = 1 + z + z ** 2 / 2 + z ** 3 / 6
+    assert np.abs(z ** 3 / 6).max() > 4e-3
+    err = np.abs(e1 - kutta * e0).max() / np.abs(e0).max()
+    assert err < 1e-10, err
+    wrong = 1 - z + z ** 2 / 2 - z ** 3 / 6                   # the other direction of time misses by ~2|z| = 0.6
+    assert np.abs(e1 - wrong * e0).max() / np.abs(e0).max() > 0.1
+
+
+@pytest.mark.parametrize("adjoint", [False, True])
+@pytest.mark.parametrize("mutation", ["stage2_F1", "stage3_quarter", "stage3_F1"])
+def test_P19f_detects_wrong_rk3_weights(mutation, adjoint):
+    e0, e1, z = _lin_inviscid_squire_step(adjoint, step=_mutated_lin_step(mutation))
+    if adjoint:
+        z = -z
+    kutta = 1 + z + z ** 2 / 2 + z ** 3 / 6
+    assert np.abs(e1 - kutta * e0).max() / np.abs(e0).max() > 1e-3
+
+
+def test_P19f_mutation_harness_reproduces_the_real_step():
+    """The mutation harness with no mutation is LinearEnsemble.step: the red results above are due to the weights alone."""
+    a = _lin_inviscid_squire_step(False)
+    b = _lin_inviscid_squire_step(False, step=_mutated_lin_step("none"))
+    assert np.array_equal(a[1], b[1])
+
+
+def test_P19g_energy_normalisation_of_B1_against_the_pinned_dns_energy():
+    """LinearEnsemble.inner carries the 1/(2V) of Eq. B.1 as the factor 0.5 on the sum over the stored
+    kx > 0 modes (a stored mode stands for the pair +-kx).  Pin: a DNS state that holds the same single-kx disturbance and
+    nothing else (U00 = W00 = 0, Poiseuille walls at rest) has, by Oracle.energy -- itself pinned by the generator's closed
+    form and by P11 -- the same energy.  P19c/P19d use inner() on both sides of their comparisons, so its constant cancels
+    there; here 0.5 -> 1.0 (or 0.25) is off by a factor 2."""
+    cfg, st, L = base_and_members(POISEUILLE_CMF, n_list=(1, 2), Eg=2)
+    o = Oracle(cfg.Nx, cfg.Ny, cfg.Nz, L.E, cfg.Re, cfg.Lx, cfg.Lz, cfg.dt, POISEUILLE_CMF)
+    v = np.zeros((L.E, o.nkx, o.nkz, o.Ny), complex)
+    eta = np.zeros_like(v)
+    for e, n in enumerate(L.n_of):
+        v[e, n], eta[e, n] = L.v[e], L.eta[e]
+    o.set_state(v, eta, np.zeros((L.E, o.Ny)), np.zeros((L.E, o.Ny)))
+    want, got = o.energy(), L.energy()
+    assert (want > 1e-6).all()
+    assert np.abs(got - want).max() < 1e-13 * want.max(), (got, want)
+    # and the cross terms: <a, b> is conjugate-symmetric and linear in b with the same constant
+    ab, ba = L.inner(0, 1), L.inner(1, 0)
+    assert abs(ab - np.conj(ba)) < 1e-15 * want.max()
+    L.v[1], L.eta[1] = L.v[0] + L.v[1], L.eta[0] + L.eta[1]
+    assert abs(L.inner(0, 1) - (L.inner(0, 0) + ab)) < 1e-14 * want.max()
