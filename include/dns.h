@@ -44,7 +44,8 @@ enum {
     DNS_ENOMEM = -2,     /* host or device allocation failed */
     DNS_ECUDA = -3,      /* CUDA runtime error or no device; sticky on the plan */
     DNS_ENONFINITE = -4, /* a member's energy is not finite (dns_diagnostics) */
-    DNS_ESTATE = -5      /* call out of order (no workspace bound, no state set) */
+    DNS_ESTATE = -5,     /* call out of order (no workspace bound, no state set) */
+    DNS_ELIMIT = -6      /* the problem is larger than the fixed capacity of dns_energy_noalloc */
 };
 
 /* kernel classes reported by dns_step_profile (north_star subsystems (1)-(4)) */
@@ -197,6 +198,40 @@ int dns_lin_energy(dns_plan* lin, double* out);
 int dns_lin_orthonormalise(dns_plan* lin);
 int dns_lin_optimals(dns_plan* lin, int nsteps, int niter, double* gains);
 int dns_lin_launches_per_step(const dns_plan* lin);
+
+/* dns_energy_noalloc -- energy_dev[E] = kinetic energy 1/(2V) int |u|^2 dV (Eq. B.1) of every member of
+ * the plan's current state: the number dns_diagnostics reports in column 0 (DNS plan) and dns_lin_energy reports
+ * (linearised plan), computed in the same order of operations.
+ *
+ * Who it is for.  The other two calls stage their result through memory carved from the workspace or through a host
+ * vector.  Some callers may not create memory at the point where they want an energy: a monitor that runs inside a
+ * time loop whose every device byte was handed out up front (a pool or caching allocator owns the GPU, or the job runs
+ * under a fixed memory budget on a shared or partitioned GPU, so a fresh device allocation can fail long into a run);
+ * code on a latency-critical path, where a device allocation or free stalls the whole GPU until earlier work has
+ * drained; and host code that is simply not allowed to call the CUDA allocator (plug-ins, callbacks).  This call
+ * allocates nothing, neither on the host nor on the device, and frees nothing.  The table of per-plane partial sums it
+ * needs between its two kernels is a fixed 512 KiB array inside the library image; every GPU that loads the library
+ * holds those 512 KiB until the process exits, used or not.
+ *
+ * Limit.  Ny * E <= DNS_NOALLOC_MAX_DOUBLES (65536; e.g. Ny = 65 with up to 1008 members).  A larger plan is refused with
+ * DNS_ELIMIT and nothing is launched: use dns_diagnostics / dns_lin_energy there.
+ *
+ * Arguments.  plan: bound and with a state (DNS or linearised); its device must be the current one.  energy_dev: DEVICE
+ * pointer to E doubles owned by the caller (a host pointer is refused with DNS_EINVAL: copying to pageable host memory
+ * would need a staging buffer).  Two kernels are enqueued on the plan's stream; the call does not synchronise, so read
+ * energy_dev in stream order.
+ *
+ * First call on a device.  It looks up where the fixed array lives on that device (once per device, remembered
+ * afterwards), which can also make the CUDA runtime load the library's code onto the device.  Make that first call
+ * during set-up, outside any stream capture.
+ *
+ * Sharing.  All plans and all calls on one GPU use the same array, and it keeps whatever the last call left in it.
+ * Every entry a call reads it has written itself first, so stale contents never reach a result.  But two calls whose
+ * kernels can run at the same time on one GPU (plans bound to different streams, or several host threads) overwrite
+ * each other's partial sums: order such calls yourself (one stream, or an event between them).
+ * Errors: DNS_EINVAL (null, host pointer), DNS_ESTATE (no workspace / no state), DNS_ELIMIT, DNS_ECUDA. */
+#define DNS_NOALLOC_MAX_DOUBLES 65536
+int dns_energy_noalloc(dns_plan* plan, double* energy_dev);
 
 /* Number of kernel launches one dns_step(1) enqueues (for bench.py's gpu_launches). */
 int dns_launches_per_step(const dns_plan* plan);

@@ -14,7 +14,8 @@ import os
 import numpy as np
 
 DNS_COUETTE, DNS_POISEUILLE_CMF = 0, 1
-DNS_OK, DNS_EINVAL, DNS_ENOMEM, DNS_ECUDA, DNS_ENONFINITE, DNS_ESTATE = 0, -1, -2, -3, -4, -5
+DNS_OK, DNS_EINVAL, DNS_ENOMEM, DNS_ECUDA, DNS_ENONFINITE, DNS_ESTATE, DNS_ELIMIT = 0, -1, -2, -3, -4, -5, -6
+DNS_NOALLOC_MAX_DOUBLES = 65536
 DNS_FORM_CONVECTIVE, DNS_FORM_ROTATIONAL = 0, 1
 DNS_COUPLING_NONE, DNS_COUPLING_STREAMWISE_MEAN = 0, 1
 DNS_NCLASS = 4
@@ -30,6 +31,7 @@ EXPORTS = ("dns_plan_create", "dns_plan_set_form", "dns_plan_set_coupling", "dns
            "dns_launches_per_step", "dns_plan_destroy", "dns_strerror",
            "dns_lin_plan_create", "dns_lin_set_base", "dns_lin_set_state", "dns_lin_get_state", "dns_lin_step",
            "dns_lin_energy", "dns_lin_orthonormalise", "dns_lin_optimals", "dns_lin_launches_per_step",
+           "dns_energy_noalloc",
            "dns_debug_fetch", "dns_debug_stage", "dns_debug_set_option", "dns_debug_fp64_peak")
 EXCHANGE_FN = ctypes.CFUNCTYPE(ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p)
 
@@ -107,6 +109,8 @@ def lib():
         L.dns_lin_optimals.restype = i
         L.dns_lin_launches_per_step.argtypes = [vp]
         L.dns_lin_launches_per_step.restype = i
+        L.dns_energy_noalloc.argtypes = [vp, dp]
+        L.dns_energy_noalloc.restype = i
         L.dns_debug_set_option.argtypes = [ctypes.c_char_p, i]
         L.dns_debug_set_option.restype = i
         L.dns_debug_fp64_peak.argtypes = [i, d, ctypes.POINTER(d)]
@@ -197,6 +201,12 @@ def dns_lin_orthonormalise(h) -> int:
 
 def dns_lin_optimals(h, nsteps: int, niter: int, gains) -> int:
     return lib().dns_lin_optimals(h, int(nsteps), int(niter), _ptr(gains))
+
+
+def dns_energy_noalloc(h, energy_dev) -> int:
+    """energy_dev: a float64 CUDA tensor of E elements that the caller made beforehand; the call itself allocates nothing
+    and does not synchronise (include/dns.h).  Works on DNS and linearised plans with Ny * E <= DNS_NOALLOC_MAX_DOUBLES."""
+    return lib().dns_energy_noalloc(h, _ptr(energy_dev))
 
 
 def dns_lin_launches_per_step(h) -> int:
@@ -381,6 +391,11 @@ class Plan:
         self._chk(st, "dns_stats_get")
         return out, n
 
+    def energy_noalloc(self, out):
+        """dns_energy_noalloc: fills `out` (float64 CUDA tensor, E elements, made by the caller beforehand) with the members'
+        kinetic energies in stream order; allocates nothing and does not synchronise."""
+        self._chk(dns_energy_noalloc(self.h, out), "dns_energy_noalloc")
+
     def debug_stage(self, stage):
         self._chk(dns_debug_stage(self.h, stage), "dns_debug_stage")
 
@@ -452,6 +467,11 @@ class LinPlan:
         out = np.empty(self.E)
         self._chk(dns_lin_energy(self.h, out), "dns_lin_energy")
         return out
+
+    def energy_noalloc(self, out):
+        """dns_energy_noalloc: fills `out` (float64 CUDA tensor, E elements, made by the caller beforehand) with the members'
+        kinetic energies in stream order; allocates nothing and does not synchronise."""
+        self._chk(dns_energy_noalloc(self.h, out), "dns_energy_noalloc")
 
     def orthonormalise(self):
         self._chk(dns_lin_orthonormalise(self.h), "dns_lin_orthonormalise")

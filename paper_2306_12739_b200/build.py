@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libdns_b200.so")
 SOURCES = ["api.cu", "plan.cu", "kernels_fft.cu", "kernels_line.cu", "kernels_y.cu", "peak_fp64.cu",
-           "kernels_lin.cu", "api_lin.cu"]
+           "kernels_lin.cu", "api_lin.cu", "no_alloc.cu"]
 HEADERS = ["dns_internal.h", "fft_codelets.cuh", "fft_consts.h", os.path.join("..", "..", "include", "dns.h"),
            os.path.join("..", "..", "include", "dns_debug.h")]
 NVCC_FLAGS = [
@@ -21,7 +21,8 @@ NVCC_FLAGS = [
 # The per-pair kernel is instantiated per member-tile shape; member independence must hold bit for bit across
 # instantiations (tests/test_gpu_parity.py::test_member_independence_bitwise), so the compiler may not choose
 # fused multiply-adds differently per instantiation: no contraction in that file (the DMMAs are explicit).
-EXTRA_FLAGS = {"kernels_y.cu": ["-fmad=false"]}
+# no_alloc.cu restates the energy kernel of kernels_y.cu and must round like it.
+EXTRA_FLAGS = {"kernels_y.cu": ["-fmad=false"], "no_alloc.cu": ["-fmad=false"]}
 
 
 def _stale() -> bool:

@@ -153,6 +153,7 @@ const char* dns_strerror(int s) {
         case DNS_ECUDA: return "CUDA error or no CUDA device";
         case DNS_ENONFINITE: return "non-finite energy";
         case DNS_ESTATE: return "call out of order (workspace not bound or state not set)";
+        case DNS_ELIMIT: return "problem exceeds the fixed capacity of the allocation-free entry point (Ny * E > 65536)";
         default: return "unknown status";
     }
 }
