@@ -132,7 +132,8 @@ int dns_set_state(dns_plan* plan, const double* vhat, const double* etahat, cons
                   const double* W00);
 
 /* dns_step -- enqueue nsteps full CN/RK3 time steps (3 stages each) on the plan's stream
- * and return without synchronising.  The 15 launches of a step are captured once into a CUDA graph (on an internal
+ * and return without synchronising.  The launches of a step (dns_launches_per_step: 15, 18 with the coupled ensemble, 21 with
+ * an exchange) are captured once into a CUDA graph (on an internal
  * stream, at the first call after dns_plan_bind) and replayed per step; a failed capture (or the test option "graph" = 0 of include/dns_debug.h) falls back to
  * direct launches with identical results.  Errors: DNS_EINVAL (nsteps < 0), DNS_ESTATE (no state), DNS_ECUDA. */
 int dns_step(dns_plan* plan, int nsteps);
@@ -181,12 +182,19 @@ int dns_stats_get(dns_plan* plan, double* out, long long* nsamples);
  *                         same grid and box, in the convective form (its transform scratch is overwritten; synchronises that
  *                         plan's stream).  Errors: DNS_EINVAL (mismatch, rotational form, bad member), DNS_ESTATE, DNS_ECUDA.
  * dns_lin_set_state / dns_lin_get_state -- host or device pointers; wall rows are set to 0; get synchronises.
- * dns_lin_step         -- enqueue nsteps steps of the forward (adjoint = 0) or adjoint (adjoint = 1) equations.
- * dns_lin_energy       -- out[E] = <q_e, q_e> (host or device); synchronises.
+ * dns_lin_step         -- enqueue nsteps steps of the forward (adjoint = 0) or adjoint (adjoint = 1) equations.  As in
+ *                         dns_step the 12 launches of a step are captured once per direction into a CUDA graph and replayed
+ *                         (identical results; direct launches if the capture fails or with the test option "graph" = 0).
+ * dns_lin_energy       -- out[E] = <q_e, q_e> (host or device); synchronises.  DNS_ENONFINITE if out is a host pointer and
+ *                         an energy is not finite (out is still filled; a device out is not inspected).
  * dns_lin_orthonormalise -- modified Gram-Schmidt in member order within every kx group, energy inner product (:417).
+ *                         A member whose energy is exactly zero (or not finite) when its turn comes, e.g. a zero vector, is
+ *                         set to zero rather than divided by zero; its energy and gain then read 0 and the other members of
+ *                         its group are unaffected.
  * dns_lin_optimals     -- the power iteration of :417: orthonormalise; niter times { nsteps forward, record the gains
  *                         E(T_opt)/E(0), nsteps adjoint from the forward final state, orthonormalise }; gains[E] (host or
  *                         device) are those of the last forward leg.  T_opt = nsteps dt_lin.  Synchronises.
+ *                         DNS_ENONFINITE as for dns_lin_energy.
  * All: DNS_EINVAL for a non-linear plan or bad arguments, DNS_ESTATE before bind / set_base / set_state, DNS_ECUDA. */
 int dns_lin_plan_create(dns_plan** out, int Nx, int Ny, int Nz, int nmodes, const int* n_list, int Eg, double Re, double Lx,
                         double Lz, double dt_lin);

@@ -311,7 +311,11 @@ class Plan:
                 def _cb(ctx, dev_buf, count, stream):                 # marshalling only: a tensor view of the buffer
                     try:
                         off = int(dev_buf) - base_ptr
-                        allreduce(ws[off:off + 8 * int(count)].view(torch.float64))
+                        # the library promises the exchange is ordered on ITS stream (include/dns.h), whatever torch's
+                        # current stream is in the thread that calls dns_step: make that stream current for the call
+                        s = torch.cuda.ExternalStream(int(stream), device=ws.device) if stream else torch.cuda.default_stream(ws.device)
+                        with torch.cuda.stream(s):
+                            allreduce(ws[off:off + 8 * int(count)].view(torch.float64))
                         return 0
                     except Exception:                                  # nothing may propagate through the C frames
                         return 1

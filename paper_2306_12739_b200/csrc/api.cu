@@ -134,6 +134,7 @@ void build_step_graph(dns_plan* p) {
 }
 
 void drop_step_graph(dns_plan* p) {
+    dns_lin_drop_graphs(p);
     if (p->graph_exec) cudaGraphExecDestroy(p->graph_exec);
     if (p->graph) cudaGraphDestroy(p->graph);
     p->graph_exec = nullptr;
@@ -438,8 +439,9 @@ int dns_diagnostics(dns_plan* p, double* out) {
     if (p->sticky != DNS_OK) return p->sticky;
     if (!p->bound || !p->has_state) return DNS_ESTATE;
     DnsDev& d = p->d;
+    std::vector<double> h;
+    try { h.resize((size_t)d.E * 6); } catch (...) { return DNS_ENOMEM; }      // nothing may throw across the ABI
     launch_diag(p, (double)p->nsteps_done * d.dt);
-    std::vector<double> h((size_t)d.E * 6);
     cudaError_t e = cudaMemcpyAsync(h.data(), d.diag, h.size() * sizeof(double), cudaMemcpyDeviceToHost, p->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(p->stream);
     if (e == cudaSuccess)
@@ -474,7 +476,8 @@ int dns_stats_get(dns_plan* p, double* out, long long* nsamples) {
     if (!p->bound) return DNS_ESTATE;
     const DnsDev& d = p->d;
     const size_t NE = (size_t)d.Ny * d.E;
-    std::vector<double> h((size_t)DNS_NSTAT * NE), t((size_t)DNS_NSTAT * NE, 0.0);
+    std::vector<double> h, t;
+    try { h.resize((size_t)DNS_NSTAT * NE); t.assign((size_t)DNS_NSTAT * NE, 0.0); } catch (...) { return DNS_ENOMEM; }
     cudaError_t e = cudaMemcpyAsync(h.data(), d.stat, h.size() * sizeof(double), cudaMemcpyDeviceToHost, p->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(p->stream);
     if (e != cudaSuccess) return cuda_status(p, e);

@@ -1,6 +1,7 @@
 // C ABI of the linearised forward / adjoint ensemble (include/dns.h, dns_lin_*; PAPER.md:296-317,
 // Appendix B).  A linear plan is a dns_plan whose spectral arrays hold one streamwise mode per member; workspace, binding
 // and destruction go through dns_plan_workspace_bytes / dns_plan_bind / dns_plan_destroy.
+#include <cmath>
 #include <vector>
 
 #include "dns_internal.h"
@@ -16,6 +17,11 @@ bool is_device_ptr(const void* q) {
     cudaPointerAttributes a;
     if (cudaPointerGetAttributes(&a, q) != cudaSuccess) { cudaGetLastError(); return false; }
     return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
+}
+bool all_finite(const double* x, int n) {
+    for (int i = 0; i < n; ++i)
+        if (!std::isfinite(x[i])) return false;
+    return true;
 }
 int check(dns_plan* p, bool need_state) {
     if (!p) return DNS_EINVAL;
@@ -34,7 +40,39 @@ void lin_stage(dns_plan* p, int s, int adjoint) {
     launch_ypair(p, s, 0);
 }
 
+// One linear step (3 stages x 4 launches) captured into a CUDA graph per direction, as dns_step does for the DNS step: at
+// the paper's size (45 disturbances) every kernel of the step lasts a few microseconds and the step is bound by
+// launch overhead.  Captured on the plan's internal stream; any failure leaves the direction on direct launches for good.
+void build_lin_graph(dns_plan* p, int adjoint) {
+    p->lin_graph_state[adjoint] = -1;
+    if (dns_option("graph") == 0) return;
+    if (cudaPeekAtLastError() != cudaSuccess) return;
+    if (!p->capture_stream && cudaStreamCreateWithFlags(&p->capture_stream, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); return; }
+    cudaStream_t user = p->stream;
+    if (cudaStreamBeginCapture(p->capture_stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { cudaGetLastError(); return; }
+    p->stream = p->capture_stream;
+    for (int s = 0; s < 3; ++s) lin_stage(p, s, adjoint);
+    p->stream = user;
+    cudaGraph_t g = nullptr;
+    if (cudaStreamEndCapture(p->capture_stream, &g) != cudaSuccess || !g) { cudaGetLastError(); return; }
+    cudaGraphExec_t ge = nullptr;
+    if (cudaGraphInstantiate(&ge, g, 0) != cudaSuccess || !ge) { cudaGetLastError(); cudaGraphDestroy(g); return; }
+    p->lin_graph[adjoint] = g;
+    p->lin_graph_exec[adjoint] = ge;
+    p->lin_graph_state[adjoint] = 1;
+}
+
 }  // namespace
+
+void dns_lin_drop_graphs(dns_plan* p) {
+    for (int a = 0; a < 2; ++a) {
+        if (p->lin_graph_exec[a]) cudaGraphExecDestroy(p->lin_graph_exec[a]);
+        if (p->lin_graph[a]) cudaGraphDestroy(p->lin_graph[a]);
+        p->lin_graph_exec[a] = nullptr;
+        p->lin_graph[a] = nullptr;
+        p->lin_graph_state[a] = 0;
+    }
+}
 
 extern "C" {
 
@@ -55,6 +93,9 @@ int dns_lin_set_base(dns_plan* lin, dns_plan* dns, int member) {
     if (dns->d.form != DNS_FORM_CONVECTIVE) return DNS_EINVAL;        // the mixed arrays must hold du/dy, dw/dy
     if (dns->sticky != DNS_OK) return dns->sticky;
     if (!dns->bound || !dns->has_state) return DNS_ESTATE;
+    // linear steps still in flight on the linear plan's stream read the base flow that is about to be rewritten
+    const cudaError_t e0 = cudaStreamSynchronize(lin->stream);
+    if (e0 != cudaSuccess) return cuda_status(lin, e0);
     // the DNS plan's transform inputs (u, w, du/dy, dw/dy of its current state) -> mixed (kx, z) arrays; their kx = 0
     // column is the streamwise-mean flow in physical z.  I8 is scratch of the DNS plan, rewritten by its next stage.
     launch_zinv(dns, dns->d.vt, dns->d.et);
@@ -112,8 +153,14 @@ int dns_lin_step(dns_plan* p, int nsteps, int adjoint) {
     const int st = check(p, true);
     if (st != DNS_OK) return st;
     if (nsteps < 0 || (adjoint != 0 && adjoint != 1)) return DNS_EINVAL;
-    for (int it = 0; it < nsteps; ++it)
-        for (int s = 0; s < 3; ++s) lin_stage(p, s, adjoint);
+    if (p->lin_graph_state[adjoint] == 0 && nsteps > 0) build_lin_graph(p, adjoint);
+    for (int it = 0; it < nsteps; ++it) {
+        if (p->lin_graph_state[adjoint] == 1) {
+            if (cudaGraphLaunch(p->lin_graph_exec[adjoint], p->stream) != cudaSuccess) return cuda_status(p, cudaGetLastError());
+        } else {
+            for (int s = 0; s < 3; ++s) lin_stage(p, s, adjoint);
+        }
+    }
     return cuda_status(p, cudaGetLastError());
 }
 
@@ -123,10 +170,12 @@ int dns_lin_energy(dns_plan* p, double* out) {
     if (!out) return DNS_EINVAL;
     if (!p->has_state) return DNS_ESTATE;
     launch_lin_energy(p, p->d.lin_scr);
+    const bool dev = is_device_ptr(out);
     cudaError_t e = cudaMemcpyAsync(out, p->d.lin_scr, p->d.E * sizeof(double),
-                                    is_device_ptr(out) ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, p->stream);
+                                    dev ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, p->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(p->stream);
-    return cuda_status(p, e);
+    if (e != cudaSuccess) return cuda_status(p, e);
+    return (!dev && !all_finite(out, p->d.E)) ? DNS_ENONFINITE : DNS_OK;
 }
 
 int dns_lin_orthonormalise(dns_plan* p) {
@@ -150,10 +199,12 @@ int dns_lin_optimals(dns_plan* p, int nsteps, int niter, double* gains) {
         if ((st = dns_lin_step(p, nsteps, 1)) != DNS_OK) return st;
         if ((st = dns_lin_orthonormalise(p)) != DNS_OK) return st;
     }
+    const bool dev = is_device_ptr(gains);
     cudaError_t e = cudaMemcpyAsync(gains, g, p->d.E * sizeof(double),
-                                    is_device_ptr(gains) ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, p->stream);
+                                    dev ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, p->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(p->stream);
-    return cuda_status(p, e);
+    if (e != cudaSuccess) return cuda_status(p, e);
+    return (!dev && !all_finite(gains, p->d.E)) ? DNS_ENONFINITE : DNS_OK;
 }
 
 int dns_lin_launches_per_step(const dns_plan* p) { return (p && p->d.lin) ? 3 * 4 : 0; }

@@ -1,7 +1,9 @@
 // Internal declarations shared by the translation units of libdns_b200 (not part of the ABI).
 #pragma once
 #include <cuda_runtime.h>
+#include <atomic>
 #include <cstddef>
+#include <mutex>
 #include <vector>
 
 #include "../../include/dns.h"
@@ -96,6 +98,10 @@ struct dns_plan {
     cudaGraph_t graph = nullptr;
     cudaGraphExec_t graph_exec = nullptr;
     int graph_state = 0;
+    // linearised ensemble: one graph per direction (0 forward, 1 adjoint) of the 12 launches of a step, same states
+    cudaGraph_t lin_graph[2] = {nullptr, nullptr};
+    cudaGraphExec_t lin_graph_exec[2] = {nullptr, nullptr};
+    int lin_graph_state[2] = {0, 0};
     int sticky = DNS_OK;
     long long nsteps_done = 0;
     long long nstat = 0;                       // samples in d.stat
@@ -130,6 +136,34 @@ inline cudaError_t dns_launch(void (*kern)(KArgs...), dim3 grid, dim3 block, siz
 }
 #endif
 
+// Dynamic shared memory above 48 KB has to be granted per kernel with cudaFuncSetAttribute.  The grant is a property of the
+// kernel ON ONE DEVICE, so the "already granted" size is remembered per device (a plan created on a second GPU of the same
+// process must set it again there), and plans driven from several host threads may reach the same kernel at once: the
+// check-and-set is under a mutex and the granted size only grows, so a smaller request can never undo a larger grant that
+// another thread's launch relies on.  One DnsSmemGrant per kernel instantiation (a function-local static at the launch site;
+// static storage = all zero).
+constexpr int DNS_MAX_DEVICES = 64;
+struct DnsSmemGrant {
+    std::atomic<size_t> have[DNS_MAX_DEVICES];
+    std::mutex m;
+};
+template <class K> inline void dns_grant_smem(K kern, size_t smem, DnsSmemGrant& g, size_t granted_at_load, bool carveout) {
+    int dev = -1;
+    const bool known = cudaGetDevice(&dev) == cudaSuccess && dev >= 0 && dev < DNS_MAX_DEVICES;
+    if (known) {
+        const size_t have = g.have[dev].load(std::memory_order_acquire);
+        if ((have ? have : granted_at_load) >= smem) return;
+    }
+    std::lock_guard<std::mutex> lock(g.m);
+    if (known) {
+        const size_t have = g.have[dev].load(std::memory_order_relaxed);
+        if ((have ? have : granted_at_load) >= smem) return;
+    }
+    cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (carveout) cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    if (known) g.have[dev].store(smem, std::memory_order_release);
+}
+
 // host precompute (plan.cu)
 int dns_host_precompute(dns_plan* p);
 bool dns_factor_len(int M, int* R1, int* R2);
@@ -159,5 +193,6 @@ void launch_lin_normalise(dns_plan* p);
 void launch_lin_energy(dns_plan* p, double* out_dev);
 void launch_lin_gs(dns_plan* p);
 void launch_lin_base(dns_plan* lin, const dns_plan* dns, int member, cudaStream_t stream);
+void dns_lin_drop_graphs(dns_plan* p);                       // api_lin.cu: the graphs hold workspace pointers and tensor maps
 int dns_create_common(dns_plan** out, int Nx, int Ny, int Nz, int E, double Re, double Lx, double Lz, double dt, int flow,
                       int nmodes, const int* n_list, int Eg);

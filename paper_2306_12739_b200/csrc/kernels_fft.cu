@@ -429,13 +429,7 @@ bool use_zreg(int Mz) {
     return dns_option("zreg") != 0 && (Mz == 24 || Mz == 36 || Mz == 48 || Mz == 72 || Mz == 96);
 }
 
-// dynamic shared memory attributes are set once per kernel and size, not per launch
-template <class K> void ensure_smem(K kern, size_t smem, size_t* have) {
-    if (*have >= smem) return;
-    cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
-    *have = smem;
-}
+// dynamic shared memory attributes are set once per kernel, device and size, not per launch (dns_grant_smem, dns_internal.h)
 
 template <int R1, int R2> void zinv_launch(dns_plan* p, const double2* vin, const double2* ein) {
     const DnsDev& d = p->d;
@@ -446,8 +440,8 @@ template <int R1, int R2> void zinv_launch(dns_plan* p, const double2* vin, cons
     while (NB > 1 && (size_t)(M + (size_t)NB * 2 * M * ET) * sizeof(double2) > 96 * 1024) --NB;
     const size_t smem = (size_t)(M + (size_t)NB * 2 * M * ET) * sizeof(double2);
     auto kern = k_zinv<R1, R2>;
-    static size_t have = 0;
-    ensure_smem(kern, smem, &have);
+    static DnsSmemGrant grant;
+    dns_grant_smem(kern, smem, grant, 0, true);
     dim3 grid((unsigned)(d.Ni * ((d.nkx + NB - 1) / NB) * ((d.E + ET - 1) / ET)), d.form == DNS_FORM_ROTATIONAL ? 6 : 5);
     dns_launch(kern, grid, dim3(256), smem, p->stream, d, vin, ein, etlog, NB);
 }
@@ -461,8 +455,8 @@ template <int R1, int R2> void zfwd_launch(dns_plan* p) {
     while (NB > 1 && (size_t)(M + (size_t)NB * M * ET) * sizeof(double2) > 96 * 1024) --NB;
     const size_t smem = (size_t)(M + (size_t)NB * M * ET) * sizeof(double2);
     auto kern = k_zfwd<R1, R2>;
-    static size_t have = 0;
-    ensure_smem(kern, smem, &have);
+    static DnsSmemGrant grant;
+    dns_grant_smem(kern, smem, grant, 0, true);
     dim3 grid((unsigned)(d.Ni * ((d.nkx + NB - 1) / NB) * ((d.E + ET - 1) / ET)), 3);
     dns_launch(kern, grid, dim3(256), smem, p->stream, d, etlog, NB);
 }

@@ -113,7 +113,10 @@ template <int EB> __global__ void __launch_bounds__(1024) k_lin_gs(DnsDev d) {
         if (threadIdx.x == 0) {
             double s = 0.0;
             for (int k = 0; k < NSL; ++k) s += red[k * EB].x;
-            coef[0] = make_double2(1.0 / sqrt(0.5 * s), 0.0);
+            // a member with exactly no energy (a zero vector) has no direction: it is set to zero instead of being divided
+            // by zero, so that it cannot turn every later member of the group into NaN; its energy then reads 0
+            const double en = 0.5 * s;
+            coef[0] = make_double2((en > 0.0 && en < 1.0e300) ? 1.0 / sqrt(en) : 0.0, 0.0);
         }
         __syncthreads();
         const double sc = coef[0].x;

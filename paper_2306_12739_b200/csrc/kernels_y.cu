@@ -779,13 +779,13 @@ int dns_ypair_encode_maps(dns_plan* p) {
     typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                   const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-    static encode_fn encode = nullptr;
-    if (!encode) {
+    static const encode_fn encode = [] {       // looked up once; the initialisation of a local static is thread-safe
         void* fn = nullptr;
         cudaDriverEntryPointQueryResult q;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) != cudaSuccess || !fn) return DNS_ECUDA;
-        encode = reinterpret_cast<encode_fn>(fn);
-    }
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) != cudaSuccess) fn = nullptr;
+        return reinterpret_cast<encode_fn>(fn);
+    }();
+    if (!encode) return DNS_ECUDA;
     const DnsDev& d = p->d;
     static_assert(sizeof(CUtensorMap) == sizeof(p->tmaps[0]), "tensor map storage");
     struct Src { void* ptr; cuuint64_t rows; } src[3] = {{d.Nh, (cuuint64_t)3 * d.Ny}, {d.vt, (cuuint64_t)d.Ny}, {d.et, (cuuint64_t)d.Ny}};
@@ -811,12 +811,8 @@ template <int NT, int NWN> static void ypair_launch(dns_plan* p, int stage, int 
 #define LAUNCH(K)                                                                                     \
     {                                                                                                 \
         auto kern = k_ypair<NT, NWN, K>;                                                              \
-        static size_t attr_smem = 0;          /* the attributes are set once per instantiation and size, not per launch */ \
-        if (attr_smem < smem) {                                                                       \
-            cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);       \
-            cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared); \
-            attr_smem = smem;                                                                         \
-        }                                                                                             \
+        static DnsSmemGrant grant;            /* the attributes are set once per instantiation, device and size, not per launch */ \
+        dns_grant_smem(kern, smem, grant, 0, true);                                                   \
         const CUtensorMap* tm = reinterpret_cast<const CUtensorMap*>(p->tmaps);                       \
         dns_launch(kern, dim3(grid), dim3(32 * KS2 * NWN), smem, p->stream, d, tm[0], tm[1], tm[2], stage, derive_only); \
     }
@@ -843,8 +839,8 @@ void launch_ypair(dns_plan* p, int stage, int derive_only) {
 void launch_mean(dns_plan* p, int stage, int derive_only, cudaStream_t stream) {
     const DnsDev& d = p->d;
     const size_t smem = (size_t)6 * d.Ny * 8 * sizeof(double);
-    static size_t attr_smem = 48 * 1024;
-    if (smem > attr_smem) { cudaFuncSetAttribute(k_mean, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr_smem = smem; }   // Ny >= 129
+    static DnsSmemGrant grant;
+    dns_grant_smem(k_mean, smem, grant, 48 * 1024, false);      // Ny >= 129
     // small ensembles: the kernel is one or a few CTAs whose serial rounds over the rows ARE its duration (and, below about
     // 16 members, longer than the z-forward + per-pair kernels it runs beside): 64 row slots finish Ny <= 66 in one round
     const int threads = (d.E <= 8 && d.Ni > 32) ? 512 : 256;

@@ -256,3 +256,37 @@ def test_line_kernel_round_variants(Nx, Nz):
             else:
                 for a, b in zip(ref, got):
                     assert np.array_equal(a, b), (name, val, form)
+
+
+def test_exchange_callback_runs_on_the_plans_stream():
+    """include/dns.h orders the exchange on the plan's stream.  The plan is bound inside a side-stream block and stepped
+    OUTSIDE it (torch's current stream is then the default one, as in bench.measure_e2e): the callback must still see the
+    plan's stream as the current stream, so that an all-reduce enqueued there is ordered between the two halves of the
+    coupled mean; the result equals the fused one-GPU path bit for bit."""
+    import torch
+    cfg = inputs.CONFIGS[2].with_E(12)
+    st = inputs.make_state(cfg)
+    ref = binding.Plan(*inputs.plan_args(cfg), coupling=COUPLED)
+    ref.set_state(st["vhat"], st["etahat"], st["U00"], st["W00"])
+    ref.step(3)
+    want = ref.get_state()
+    ref.close()
+
+    side = torch.cuda.Stream()
+    seen = []
+
+    def allreduce(t):
+        seen.append(torch.cuda.current_stream().cuda_stream)
+        t.mul_(1.0)                                           # a device operation enqueued on the current stream
+
+    with torch.cuda.stream(side):
+        plan = binding.Plan(*inputs.plan_args(cfg), coupling=COUPLED, allreduce=allreduce)
+        plan.set_state(st["vhat"], st["etahat"], st["U00"], st["W00"])
+    assert torch.cuda.current_stream().cuda_stream != side.cuda_stream
+    plan.step(3)
+    got = plan.get_state()
+    assert len(seen) == 9 and all(s == side.cuda_stream for s in seen), (seen, side.cuda_stream)
+    for a, b in zip(want, got):
+        assert np.array_equal(a, b)
+    plan.close()
+    torch.cuda.synchronize()

@@ -137,3 +137,49 @@ def test_linear_error_paths():
     assert binding.dns_lin_step(lin.h, 1, 2) in (binding.DNS_ESTATE, binding.DNS_EINVAL)
     for p in (lin, dns, rot, other):
         p.close()
+
+
+def test_gram_schmidt_with_a_zero_member_stays_finite():
+    """A member with no energy has no direction: dns_lin_orthonormalise sets it to zero instead of dividing by zero, the
+    other members of its kx group come out exactly as if it were not there, and every call still returns DNS_OK."""
+    cfg = inputs.Config(1, inputs.COUETTE, 400.0, 1.75 * PI, 1.2 * PI, 16, 25, 16, 1, 0.02, 1, 0.3, 0, box=3)
+    dns, lin, o = setup(cfg, [1, 2], 4, 0.1)
+    v, eta = lin.get_state()
+    v[1], eta[1] = 0.0, 0.0                                   # second member of the first group
+    lin.set_state(v, eta)
+    lin.orthonormalise()
+    gv, ge = lin.get_state()
+    en = lin.energy()
+    assert np.isfinite(gv).all() and np.isfinite(ge).all() and np.isfinite(en).all()
+    assert en[1] == 0.0 and np.abs(np.delete(en, 1) - 1.0).max() < 1e-12
+    # the oracle on the same vectors without the zero member (3 + 4 members would not fit its equal groups: group 0 alone)
+    o3 = LinearEnsemble(cfg.Nx, cfg.Ny, cfg.Nz, [1], 3, cfg.Re, cfg.Lx, cfg.Lz, 0.1, cfg.flow)
+    o3.set_state(v[[0, 2, 3]], eta[[0, 2, 3]])
+    o3.orthonormalise()
+    assert field_err(gv[[0, 2, 3]], o3.v) < 1e-11 and field_err(ge[[0, 2, 3]], o3.eta) < 1e-11
+    lin.step(1, False)                                        # and it keeps stepping
+    assert np.isfinite(lin.energy()).all()
+    lin.close()
+    dns.close()
+
+
+def test_linear_step_graph_replay_equals_direct_launches_bitwise():
+    """dns_lin_step replays one CUDA graph per direction; with the test option "graph" = 0 it launches directly.  Same bits,
+    forward and adjoint, also after the base flow has been replaced (the graphs hold pointers, not contents)."""
+    cfg = inputs.Config(1, inputs.COUETTE, 400.0, 1.75 * PI, 1.2 * PI, 16, 33, 16, 2, 0.02, 1, 0.3, 0, box=3)
+    outs = []
+    for graph in (-1, 0):
+        assert binding.dns_debug_set_option("graph", graph) == binding.DNS_OK
+        try:
+            dns, lin, o = setup(cfg, [1, 2, 3], 5, 5 * cfg.dt, seed_member=1)
+            lin.step(3, False)
+            lin.step(2, True)
+            lin.set_base(dns, 0)
+            lin.step(2, False)
+            outs.append(lin.get_state())
+            lin.close()
+            dns.close()
+        finally:
+            binding.dns_debug_set_option("graph", -1)
+    for a, b in zip(*outs):
+        assert np.array_equal(a, b)

@@ -441,3 +441,47 @@ def test_plan_on_a_non_default_stream():
             plan.close()
     for a, b in zip(*outs):
         assert np.array_equal(a, b)
+
+
+def test_four_plans_on_four_host_threads_equal_the_serial_run_bitwise():
+    """One plan per host thread is the supported concurrent use (bench.measure_e2e drives four).  Four threads each create,
+    bind (own stream), load and step their own plan for 50 steps at the same time -- different grids, so that they reach
+    different kernel instantiations and shared-memory grants concurrently -- and every final state equals, bit for bit, the
+    one the same plan produces when run alone."""
+    import threading
+    import torch
+
+    cfgs = [inputs.CONFIGS[1],
+            inputs.CONFIGS[2].with_E(8),
+            inputs.Config(3, inputs.POISEUILLE_CMF, 2000.0, 1.75 * PI, 1.2 * PI, 24, 41, 16, 5, 0.01, 1, 0.2, 0, box=3),
+            inputs.Config(1, inputs.COUETTE, 400.0, 1.75 * PI, 1.2 * PI, 16, 129, 24, 3, 0.01, 1, 0.2, 0, box=3)]
+    states = [inputs.make_state(c) for c in cfgs]
+
+    def run(i, out, stream=None):
+        try:
+            with torch.cuda.stream(stream if stream is not None else torch.cuda.current_stream()):
+                p = binding.Plan(*inputs.plan_args(cfgs[i]))
+                st = states[i]
+                p.set_state(st["vhat"], st["etahat"], st["U00"], st["W00"])
+                for _ in range(10):
+                    p.step(5)
+                out[i] = p.get_state() + (p.diagnostics(),)
+                p.close()
+        except Exception as exc:                              # surfaces in the main thread
+            out[i] = exc
+
+    serial = [None] * 4
+    for i in range(4):
+        run(i, serial)
+    for rep in range(2):
+        par = [None] * 4
+        threads = [threading.Thread(target=run, args=(i, par, torch.cuda.Stream())) for i in range(4)]
+        for t in threads:
+            t.start()
+        for t in threads:
+            t.join()
+        for i in range(4):
+            assert not isinstance(par[i], Exception) and not isinstance(serial[i], Exception), (par[i], serial[i])
+            for a, b in zip(serial[i], par[i]):
+                assert np.array_equal(a, b), (rep, i)
+    torch.cuda.synchronize()
