@@ -198,6 +198,9 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true",
                     help="skip the threaded end-to-end measurement (for runs under ncu only: `e2e` is then null)")
+    ap.add_argument("--no-extras", action="store_true",
+                    help="skip the `other_configs` (configs 1-3 and the config-5 sweep, 20 steps each) and `rows` (linearised "
+                         "ensemble, optimal-disturbance loop, coupled step, statistics) blocks of the default line")
     ap.add_argument("--sweep", action="store_true",
                     help="BASELINE config 5: one JSON line per ensemble size E in inputs.SWEEP_E (per-kernel times and "
                          "roofline fractions versus E); not the default bench line")
@@ -237,27 +240,31 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    def measure(cfg, cfg_all, st, rot):
-        """Device-resident timing of args.steps steps + per-kernel-class durations, one form of the nonlinear term."""
+    def measure(cfg, cfg_all, st, rot, steps=None, warmup=None, coupling=None):
+        """Device-resident timing of `steps` (default args.steps) steps + per-kernel-class durations, one form of the
+        nonlinear term; coupling: dns_plan_set_coupling mode (row f2) or None."""
+        steps = args.steps if steps is None else steps
+        warmup = args.warmup if warmup is None else warmup
         plan = binding.Plan(*inputs.plan_args(cfg), device=f"cuda:{local}",
-                            form=binding.DNS_FORM_ROTATIONAL if rot else binding.DNS_FORM_CONVECTIVE)
+                            form=binding.DNS_FORM_ROTATIONAL if rot else binding.DNS_FORM_CONVECTIVE,
+                            coupling=binding.DNS_COUPLING_NONE if coupling is None else coupling)
         plan.set_state(st["vhat"], st["etahat"], st["U00"], st["W00"])
         stream = torch.cuda.current_stream()
-        plan.step(args.warmup)
+        plan.step(warmup)
         barrier()
         sampler = ClockSampler(local)
         sampler.start()
         ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         ev0.record(stream)
-        plan.step(args.steps)
+        plan.step(steps)
         ev1.record(stream)
         barrier()
         ms = ev0.elapsed_time(ev1)
         clocks = sampler.stop()
         ms_max = shard.max_over_ranks(ms) if world > 1 else ms
-        value = cfg_all.E * args.steps / (ms_max * 1e-3)
+        value = cfg_all.E * steps / (ms_max * 1e-3)
         # per-kernel-class durations with CUDA events on the same stream (live, same state)
-        nprof = min(max(args.steps // 10, 3), 20)
+        nprof = min(max(steps // 10, 3), 20)
         prof = plan.step_profile(nprof)
         counts = workload_counts(cfg, cfg.E, rot)
         kernels = {}
@@ -350,6 +357,95 @@ def main():
                 "note": "dns_set_state(host pinned) + dns_step(1) + dns_get_state(host pinned) per step and member chunk; "
                         "%d chunks of members on their own plans, streams and host threads" % len(work)}
 
+    def other_configs():
+        """The other BASELINE configs and the config-5 sweep in short form (north_star: "all five configs"): 20 timed steps
+        each after 5 warm-up steps, convective form, same timing and per-class fractions as the headline."""
+        out = []
+        todo = [(f"config{c}", inputs.CONFIGS[c]) for c in (1, 2, 3) if c != args.config]
+        todo += [(f"config5_E{E}", inputs.CONFIGS[5].with_E(E)) for E in inputs.SWEEP_E]
+        for tag, c in todo:
+            st_ = inputs.make_state(c)
+            plan, value, ms_max, _, kernels = measure(c, c, st_, False, steps=20, warmup=5)
+            out.append({"tag": tag, "workload": c.name, "value": value, "unit": UNIT, "ms_per_step": ms_max / 20,
+                        "steps": 20, "launches_per_step": plan.launches_per_step(), "workspace_MB": plan.workspace_bytes / 1e6,
+                        "frac": {k: round(v["frac"], 4) for k, v in kernels.items()},
+                        "us_per_launch": {k: round(v["us_per_launch"], 2) for k, v in kernels.items()}})
+            plan.close()
+        return out
+
+    def timed(fn, stream):
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        ev0.record(stream)
+        fn()
+        ev1.record(stream)
+        torch.cuda.synchronize()
+        return ev0.elapsed_time(ev1)
+
+    def rows_block(cfg4, st4, base_value):
+        """One device-timed measurement for each SURVEY.md 8(f) row that is not the headline: the linearised forward /
+        adjoint ensemble at the paper's size (48 x 65 x 48, 45 disturbances, t_f = 5), one
+        optimal-disturbance loop, the coupled ensemble's cost over the uncoupled step, and dns_stats_accumulate."""
+        stream = torch.cuda.current_stream()
+        rows = {}
+        c2 = cfg4.with_E(2)
+        s2 = inputs.make_state(c2)
+        dns = binding.Plan(*inputs.plan_args(c2), device=f"cuda:{local}")
+        dns.set_state(s2["vhat"], s2["etahat"], s2["U00"], s2["W00"])
+        n_list, Eg = [1, 2, 3], 15
+        lin = binding.LinPlan(c2.Nx, c2.Ny, c2.Nz, n_list, Eg, c2.Re, c2.Lx, c2.Lz, 5 * c2.dt, device=f"cuda:{local}")
+        lin.set_base(dns, 1)
+        pert = inputs.make_broadband_state(c2.with_E(lin.E), range(20, 20 + lin.E))
+        lin.set_state(np.stack([pert["vhat"][e, n_list[e // Eg]] for e in range(lin.E)]),
+                      np.stack([pert["etahat"][e, n_list[e // Eg]] for e in range(lin.E)]))
+        lin.orthonormalise()
+        # algorithmic bytes of one linear stage: z inverse 5 S + 8 I, pointwise vector 8 I + 3 I, z forward 3 I + 3 S,
+        # per-pair kernel 13 S + the matrices of the 3 kx rows; S, I = one spectral / mixed field with ONE kx row
+        Ni, nkz, Mz = c2.Ny - 2, c2.Nz - 1, 3 * c2.Nz // 2
+        S, I = Ni * nkz * 16.0 * lin.E, Ni * Mz * 16.0 * lin.E
+        Kh, Kho = (Ni + 1) // 2, Ni // 2
+        mats = 3 * (Kh * Kh + Kho * Kho) * 8.0 * len(n_list) * (c2.Nz // 2)
+        stage_bytes = 21 * S + 22 * I + mats
+        nlin = 50
+        for adj, tag in ((False, "lin_step_forward"), (True, "lin_step_adjoint")):
+            lin.step(5, adj)
+            ms = timed(lambda: lin.step(nlin, adj), stream)
+            rows[tag] = {"value": lin.E * nlin / (ms * 1e-3), "unit": UNIT, "ms_per_step": ms / nlin, "members": lin.E,
+                         "launches_per_step": binding.dns_lin_launches_per_step(lin.h),
+                         "alg_bytes_per_step": 3 * stage_bytes, "GBps": 3 * stage_bytes * nlin / (ms * 1e-3) * 1e-9,
+                         "frac_hbm": 3 * stage_bytes * nlin / (ms * 1e-3) * 1e-9 / hbm_peak,
+                         "workload": f"{c2.Nx}x{c2.Ny}x{c2.Nz}, kx modes {n_list} x {Eg} disturbances, dt_lin = 5 dt"}
+            lin.orthonormalise()
+        nopt, niter = 20, 2
+        lin.optimals(2, 1)
+        t0 = time.perf_counter()
+        gains = lin.optimals(nopt, niter)                     # synchronises at its end
+        wall = time.perf_counter() - t0
+        rows["lin_optimals"] = {"ms": wall * 1e3, "nsteps": nopt, "niter": niter,
+                                "lin_steps_total": 2 * nopt * niter, "ms_per_lin_step": wall * 1e3 / (2 * nopt * niter),
+                                "max_gain": float(np.max(gains)),
+                                "note": "orthonormalise + niter x (nsteps forward, energies, nsteps adjoint, orthonormalise)"}
+        ms = timed(lambda: [lin.orthonormalise() for _ in range(10)], stream)
+        rows["lin_orthonormalise"] = {"ms": ms / 10, "members": lin.E, "groups": len(n_list)}
+        lin.close()
+        dns.close()
+        # coupled ensemble (row f2) on the headline workload: the same 20 steps with dns_plan_set_coupling
+        plan, value, ms_max, _, _ = measure(cfg4, cfg4, st4, False, steps=20, warmup=5,
+                                            coupling=binding.DNS_COUPLING_STREAMWISE_MEAN)
+        rows["coupled_step"] = {"value": value, "unit": UNIT, "ms_per_step": ms_max / 20,
+                                "launches_per_step": plan.launches_per_step(),
+                                "cost_over_uncoupled": base_value / value - 1.0, "workload": cfg4.name}
+        # one-point statistics (row f4) of the same plan's state: reads u, v, w of every member once
+        plan.stats_reset()
+        plan.stats_accumulate()
+        ms = timed(lambda: [plan.stats_accumulate() for _ in range(20)], stream)
+        P = (cfg4.Nx // 2) * (cfg4.Nz - 1)
+        sb = 3 * cfg4.Ny * P * 16.0 * cfg4.E
+        rows["stats_accumulate"] = {"us_per_call": ms * 1e3 / 20, "alg_bytes_per_call": sb,
+                                    "GBps": sb / (ms * 1e-3 / 20) * 1e-9, "frac_hbm": sb / (ms * 1e-3 / 20) * 1e-9 / hbm_peak}
+        plan.close()
+        return rows
+
     for E_gpu in sizes:
         if args.sweep:
             args.steps, args.warmup = 50, 5                  # BASELINE config 5: 50 steps per ensemble size
@@ -388,6 +484,12 @@ def main():
                                   "clocks": r["clocks"], "roofline": r["roofline"], "kernels": r["kernels"],
                                   "note": "same workload, steps and timing with dns_plan_set_form(DNS_FORM_ROTATIONAL), "
                                           "SURVEY.md 8(f) row f1"}
+        if world == 1 and not args.sweep and not args.no_extras and args.config == 4 and not args.members:
+            try:
+                line["other_configs"] = other_configs()
+                line["rows"] = rows_block(cfg, st, head["value"])
+            except Exception as exc:                              # the headline line must still be printed
+                line["extras_error"] = repr(exc)
         if rank == 0 and world == 1 and not args.no_cpu_baseline and not args.sweep:
             line["cpu_baseline"] = cpu_baseline(base)
         if rank == 0:
