@@ -198,6 +198,9 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true",
                     help="skip the threaded end-to-end measurement (for runs under ncu only: `e2e` is then null)")
+    ap.add_argument("--opt", action="append", default=[], metavar="NAME=VALUE",
+                    help="dns_debug_set_option before the plans are created (experiments, e.g. --opt line_96=1); "
+                         "the options used are recorded in config.options")
     ap.add_argument("--no-extras", action="store_true",
                     help="skip the `other_configs` (configs 1-3 and the config-5 sweep, 20 steps each) and `rows` (linearised "
                          "ensemble, optimal-disturbance loop, coupled step, statistics) blocks of the default line")
@@ -222,6 +225,10 @@ def main():
     torch.cuda.set_device(local)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    for o in args.opt:
+        name, val = o.split("=", 1)
+        if binding.dns_debug_set_option(name, int(val)) != binding.DNS_OK:
+            raise SystemExit(f"unknown option {name}")
     base = inputs.CONFIGS[5 if args.sweep else args.config]
     sizes = list(inputs.SWEEP_E) if args.sweep else [args.members or base.E]
     hbm_peak, peak_src = measured_peaks()
@@ -474,7 +481,7 @@ def main():
                        "parallelism": f"member-shards x{world} (no collective in dns_step)",
                        "l2_policy": "working set %.0f MB per GPU > 126 MB L2 (no flush needed)" % (head["ws"] / 1e6)
                        if head["ws"] > 2 * 126e6 else "working set fits L2; not flushed between steps (stated)",
-                       "input_sha256": st["sha256"][:16]},
+                       "input_sha256": st["sha256"][:16], **({"options": args.opt} if args.opt else {})},
             "clocks": head["clocks"], "e2e": e2e, "gpu_launches": args.steps * head["launches"],
             "roofline": head["roofline"], "kernels": head["kernels"], "fp64_peak": fp64,
         }
@@ -484,7 +491,7 @@ def main():
                                   "clocks": r["clocks"], "roofline": r["roofline"], "kernels": r["kernels"],
                                   "note": "same workload, steps and timing with dns_plan_set_form(DNS_FORM_ROTATIONAL), "
                                           "SURVEY.md 8(f) row f1"}
-        if world == 1 and not args.sweep and not args.no_extras and args.config == 4 and not args.members:
+        if world == 1 and not args.sweep and not args.no_extras and args.config == 4 and not args.members and not args.opt:
             try:
                 line["other_configs"] = other_configs()
                 line["rows"] = rows_block(cfg, st, head["value"])

@@ -33,8 +33,10 @@ def _stale() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False, extra_flags=()) -> str:
-    """extra_flags: additional nvcc flags for experiments (e.g. -DDNS_YP_REGCAP=112); the product build passes none."""
+def build(force: bool = False, verbose: bool = False, extra_flags=(), drop_file_flags=()) -> str:
+    """extra_flags: additional nvcc flags for experiments (e.g. -DDNS_YP_REGCAP=112); drop_file_flags: sources whose
+    EXTRA_FLAGS are left out (experiment: `--contract=kernels_y.cu` measures that file with fused multiply-adds).  The
+    product build passes neither."""
     if not force and not _stale():
         return LIB
     nvcc = "/usr/local/cuda/bin/nvcc"
@@ -45,7 +47,8 @@ def build(force: bool = False, verbose: bool = False, extra_flags=()) -> str:
     for s in SOURCES:
         o = os.path.join(HERE, "build", s.replace(".cu", ".o"))
         objs.append(o)
-        cmd = [nvcc, *NVCC_FLAGS, *EXTRA_FLAGS.get(s, []), *extra_env, "-c", os.path.join(CSRC, s), "-o", o]
+        file_flags = [] if s in drop_file_flags else EXTRA_FLAGS.get(s, [])
+        cmd = [nvcc, *NVCC_FLAGS, *file_flags, *extra_env, "-c", os.path.join(CSRC, s), "-o", o]
         procs.append((s, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
     log = []
     for s, p in procs:
@@ -68,4 +71,5 @@ def build(force: bool = False, verbose: bool = False, extra_flags=()) -> str:
 
 if __name__ == "__main__":
     print(build(force="--force" in sys.argv, verbose="-v" in sys.argv,
-                extra_flags=[a for a in sys.argv[1:] if a.startswith("-D") or a.startswith("-X") or a.startswith("--max")]))
+                extra_flags=[a for a in sys.argv[1:] if a.startswith("-D") or a.startswith("-X") or a.startswith("--max")],
+                drop_file_flags=[a.split("=", 1)[1] for a in sys.argv[1:] if a.startswith("--contract=")]))

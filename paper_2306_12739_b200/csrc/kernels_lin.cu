@@ -8,7 +8,7 @@
 //                    adjoint (B.5, reversed time, reading L1)  N_i = -(U.grad) lam_i - U_j d_i lam_j
 //   k_lin_base     : copies the kx = 0 column of one member of a DNS plan's mixed arrays = the base flow and its gradient
 //   k_lin_energy   : E_e = (1/2) sum_m sum_j w_j (|u|^2 + |v|^2 + |w|^2)                                  (B.1)
-//   k_lin_gs       : modified Gram-Schmidt in member order within each kx group, energy inner product     (:417)
+//   k_lin_gs_*     : modified Gram-Schmidt in member order within each kx group, energy inner product     (:417)
 #include "dns_internal.h"
 
 namespace {
@@ -88,81 +88,84 @@ __global__ void k_lin_energy_rows(DnsDev d, const double* __restrict__ part, dou
     out[e] = s;
 }
 
-// ---- modified Gram-Schmidt (reading L4): one CTA per kx group; the vectors are (v, eta) with their u, w (linear in the
-// state), the inner product is (1/2) sum_{m,j} w_j (conj(u_a) u_b + conj(v_a) v_b + conj(w_a) w_b).
-// Threads = EB member lanes x NSL element slots; partial sums are added in ascending slot order (deterministic).
-template <int EB> __global__ void __launch_bounds__(1024) k_lin_gs(DnsDev d) {
-    constexpr int NSL = 1024 / EB;
-    __shared__ double2 red[1024];
-    __shared__ double2 coef[EB];
-    const int g = blockIdx.x, bl = threadIdx.x % EB, slot = threadIdx.x / EB;
-    const int e_first = g * d.Eg, L = d.Ny * d.P;
-    double2* X[4] = {d.vt, d.et, d.uh, d.wh};
-    for (int a = 0; a < d.Eg; ++a) {
-        const int ea = e_first + a;
-        // norm of member a (all threads: lane 0 of every slot sums, the others idle)
+// ---- modified Gram-Schmidt (reading L4) in member order within each kx group.  The vectors are (v, eta) with
+// their u, w (linear in the state); the inner product is (1/2) sum_{m,j} w_j (conj(u_a) u_b + conj(v_a) v_b + conj(w_a) w_b).
+// The loop over a is serial by nature; everything inside one a is not: the products of member a with itself and with all
+// later members b of its group are independent, and so are their updates.  Two launches per a over a grid of
+// (kx groups) x (NCH chunks of the Ny P elements of a vector):
+//   k_lin_gs_dots   : part[g][chunk][b] = sum over the chunk of w_j conj(x_a) . x_b for b = a .. Eg-1 (b = a: the norm)
+//   k_lin_gs_update : every CTA adds the chunk sums in ascending order (the same numbers in every CTA), then in its own chunk
+//                     x_b -= (<x_a, x_b> / <x_a, x_a>) x_a for b > a and, once all of those have read x_a, x_a /= |x_a|
+// which is the modified Gram-Schmidt step with the division by |x_a| moved out of the inner product.  Threads = EB member
+// lanes x (256 / EB) element slots; slot and chunk sums are added in fixed ascending order (deterministic).  A member with
+// exactly zero (or non-finite) energy has no direction: it is set to zero instead of being divided by zero, so that it cannot
+// turn the later members of its group into NaN; its energy then reads 0.
+// (Until round 3 this was one 1024-thread CTA per kx group: 2.08 ms for 3 x 15 vectors at 48 x 65 x 48 on 3 of 148 SMs.)
+constexpr int GS_THREADS = 256;
+__device__ __forceinline__ int gs_lanes(int Eg) { int b = 1; while (b < Eg && b < 32) b <<= 1; return b; }
+
+__global__ void __launch_bounds__(GS_THREADS) k_lin_gs_dots(DnsDev d, int a, int NCH, double2* __restrict__ part) {
+    __shared__ double2 red[GS_THREADS];
+    const int g = blockIdx.x, ch = blockIdx.y, EB = gs_lanes(d.Eg), nslot = GS_THREADS / EB;
+    const int bl = threadIdx.x % EB, slot = threadIdx.x / EB;
+    const int L = d.Ny * d.P, CL = (L + NCH - 1) / NCH, i0 = ch * CL, i1 = min(L, i0 + CL);
+    const int e_first = g * d.Eg, ea = e_first + a;
+    for (int b0 = a; b0 < d.Eg; b0 += EB) {
+        const int b = b0 + bl, eb = e_first + b;
         double2 acc = make_double2(0.0, 0.0);
-        if (bl == 0)
-            for (int i = slot; i < L; i += NSL) {
-                const size_t gi = (size_t)i * d.E + ea;
-                const double2 u = d.uh[gi], v = d.vt[gi], w = d.wh[gi];
-                acc.x += d.w[i / d.P] * (u.x * u.x + u.y * u.y + v.x * v.x + v.y * v.y + w.x * w.x + w.y * w.y);
+        if (b < d.Eg)
+            for (int i = i0 + slot; i < i1; i += nslot) {
+                const size_t ga = (size_t)i * d.E + ea, gb = (size_t)i * d.E + eb;
+                const double wj = d.w[i / d.P];
+                const double2 ua = d.uh[ga], va = d.vt[ga], wa = d.wh[ga], ub = d.uh[gb], vb = d.vt[gb], wb = d.wh[gb];
+                acc.x += wj * (ua.x * ub.x + ua.y * ub.y + va.x * vb.x + va.y * vb.y + wa.x * wb.x + wa.y * wb.y);      // conj(a) b
+                acc.y += wj * (ua.x * ub.y - ua.y * ub.x + va.x * vb.y - va.y * vb.x + wa.x * wb.y - wa.y * wb.x);
             }
         red[slot * EB + bl] = acc;
         __syncthreads();
-        if (threadIdx.x == 0) {
-            double s = 0.0;
-            for (int k = 0; k < NSL; ++k) s += red[k * EB].x;
-            // a member with exactly no energy (a zero vector) has no direction: it is set to zero instead of being divided
-            // by zero, so that it cannot turn every later member of the group into NaN; its energy then reads 0
-            const double en = 0.5 * s;
-            coef[0] = make_double2((en > 0.0 && en < 1.0e300) ? 1.0 / sqrt(en) : 0.0, 0.0);
+        if (slot == 0 && b < d.Eg) {
+            double2 t = make_double2(0.0, 0.0);
+            for (int k = 0; k < nslot; ++k) { t.x += red[k * EB + bl].x; t.y += red[k * EB + bl].y; }
+            part[((size_t)g * NCH + ch) * d.Eg + b] = t;
         }
         __syncthreads();
-        const double sc = coef[0].x;
-        for (int i = threadIdx.x; i < L; i += 1024) {
-            const size_t gi = (size_t)i * d.E + ea;
+    }
+}
+
+__global__ void __launch_bounds__(GS_THREADS) k_lin_gs_update(DnsDev d, int a, int NCH, const double2* __restrict__ part) {
+    const int g = blockIdx.x, ch = blockIdx.y, EB = gs_lanes(d.Eg), nslot = GS_THREADS / EB;
+    const int bl = threadIdx.x % EB, slot = threadIdx.x / EB;
+    const int L = d.Ny * d.P, CL = (L + NCH - 1) / NCH, i0 = ch * CL, i1 = min(L, i0 + CL);
+    const int e_first = g * d.Eg, ea = e_first + a;
+    double2* X[4] = {d.vt, d.et, d.uh, d.wh};
+    double saa = 0.0;
+    for (int k = 0; k < NCH; ++k) saa += part[((size_t)g * NCH + k) * d.Eg + a].x;
+    const double en = 0.5 * saa;                              // energy of x_a (B.1)
+    const bool ok = en > 0.0 && en < 1.0e300;
+    for (int b0 = a + 1; b0 < d.Eg; b0 += EB) {
+        const int b = b0 + bl, eb = e_first + b;
+        if (b >= d.Eg || !ok) continue;
+        double2 sab = make_double2(0.0, 0.0);
+        for (int k = 0; k < NCH; ++k) { const double2 t = part[((size_t)g * NCH + k) * d.Eg + b]; sab.x += t.x; sab.y += t.y; }
+        const double2 c = make_double2(sab.x / saa, sab.y / saa);          // <x_a, x_b> / <x_a, x_a>
+        for (int i = i0 + slot; i < i1; i += nslot) {
+            const size_t ga = (size_t)i * d.E + ea, gb = (size_t)i * d.E + eb;
 #pragma unroll
-            for (int f = 0; f < 4; ++f) X[f][gi] = cscale(sc, X[f][gi]);
-        }
-        __syncthreads();
-        // projections of the later members of the group on member a, EB members at a time
-        for (int b0 = a + 1; b0 < d.Eg; b0 += EB) {
-            const int b = b0 + bl, eb = e_first + b;
-            acc = make_double2(0.0, 0.0);
-            if (b < d.Eg)
-                for (int i = slot; i < L; i += NSL) {
-                    const size_t ga = (size_t)i * d.E + ea, gb = (size_t)i * d.E + eb;
-                    const double wj = d.w[i / d.P];
-                    const double2 ua = d.uh[ga], va = d.vt[ga], wa = d.wh[ga], ub = d.uh[gb], vb = d.vt[gb], wb = d.wh[gb];
-                    // conj(a) * b
-                    acc.x += wj * (ua.x * ub.x + ua.y * ub.y + va.x * vb.x + va.y * vb.y + wa.x * wb.x + wa.y * wb.y);
-                    acc.y += wj * (ua.x * ub.y - ua.y * ub.x + va.x * vb.y - va.y * vb.x + wa.x * wb.y - wa.y * wb.x);
-                }
-            red[slot * EB + bl] = acc;
-            __syncthreads();
-            if (slot == 0) {
-                double2 s = make_double2(0.0, 0.0);
-                for (int k = 0; k < NSL; ++k) { s.x += red[k * EB + bl].x; s.y += red[k * EB + bl].y; }
-                coef[bl] = make_double2(0.5 * s.x, 0.5 * s.y);
+            for (int f = 0; f < 4; ++f) {
+                const double2 xa = X[f][ga];
+                double2 xb = X[f][gb];
+                xb.x -= c.x * xa.x - c.y * xa.y;
+                xb.y -= c.x * xa.y + c.y * xa.x;
+                X[f][gb] = xb;
             }
-            __syncthreads();
-            if (b < d.Eg) {
-                const double2 c = coef[bl];
-                for (int i = slot; i < L; i += NSL) {
-                    const size_t ga = (size_t)i * d.E + ea, gb = (size_t)i * d.E + eb;
+        }
+    }
+    __syncthreads();                                          // every read of x_a in this chunk is done
+    const double sc = ok ? 1.0 / sqrt(en) : 0.0;
+    for (int i = i0 + threadIdx.x; i < i1; i += GS_THREADS) {
+        const size_t ga = (size_t)i * d.E + ea;
 #pragma unroll
-                    for (int f = 0; f < 4; ++f) {
-                        const double2 xa = X[f][ga];
-                        double2 xb = X[f][gb];
-                        xb.x -= c.x * xa.x - c.y * xa.y;
-                        xb.y -= c.x * xa.y + c.y * xa.x;
-                        X[f][gb] = xb;
-                    }
-                }
-            }
-            __syncthreads();
-        }
+        for (int f = 0; f < 4; ++f) X[f][ga] = cscale(sc, X[f][ga]);
     }
 }
 
@@ -186,8 +189,14 @@ void launch_lin_energy(dns_plan* p, double* out_dev) {
 }
 void launch_lin_gs(dns_plan* p) {
     const DnsDev& d = p->d;
-    if (d.Eg <= 4) k_lin_gs<4><<<d.nmodes, 1024, 0, p->stream>>>(d);
-    else if (d.Eg <= 8) k_lin_gs<8><<<d.nmodes, 1024, 0, p->stream>>>(d);
-    else if (d.Eg <= 16) k_lin_gs<16><<<d.nmodes, 1024, 0, p->stream>>>(d);
-    else k_lin_gs<32><<<d.nmodes, 1024, 0, p->stream>>>(d);
+    // chunk sums live in the [Ny][E] part of lin_scr (shared with the energy's plane sums, same stream): E NCH complex
+    int NCH = d.Ny / 2;
+    if (NCH > 32) NCH = 32;
+    if (NCH < 1) NCH = 1;
+    double2* part = reinterpret_cast<double2*>(d.lin_scr + 2 * (size_t)d.E);
+    const dim3 grid(d.nmodes, NCH);
+    for (int a = 0; a < d.Eg; ++a) {
+        k_lin_gs_dots<<<grid, GS_THREADS, 0, p->stream>>>(d, a, NCH, part);
+        k_lin_gs_update<<<grid, GS_THREADS, 0, p->stream>>>(d, a, NCH, part);
+    }
 }

@@ -703,11 +703,14 @@ __global__ void k_diag_rows(DnsDev d, const double* __restrict__ part, double t)
 }
 
 // one-point statistics of the current state (row f4): Parseval sums over the retained modes, added to the running sums
+// grid = (Ny, ceil(E / EB)) with EB = 32 member lanes at most: 8 mode slots per member block and enough CTAs to fill the GPU
+// (one CTA per plane walked all P modes of 256 members with one slot: 65 CTAs, 0.20 of the HBM roofline on config 4)
 __global__ void __launch_bounds__(256) k_stats(DnsDev d) {
     __shared__ double sm[4 * 256];
-    const int j = blockIdx.x, EB = member_block(d.E);
+    const int j = blockIdx.x, EB = min(member_block(d.E), 32);
     const size_t NE = (size_t)d.Ny * d.E;
-    for (int e0 = 0; e0 < d.E; e0 += EB) {
+    {
+        const int e0 = blockIdx.y * EB;
         double s[4];
         plane_mode_sums<4>(d, j, 1, sm, [&](int p, size_t gi, double* a) {
             const double2 u = d.uh[gi], v = d.vt[gi], w = d.wh[gi];
@@ -864,7 +867,11 @@ void launch_mean_in(dns_plan* p, const double* U, const double* W) {
 void launch_mean_out(dns_plan* p, double* U, double* W) {
     k_mean_out<<<(p->d.E + 127) / 128, 128, 0, p->stream>>>(p->d, U, W);
 }
-void launch_stats(dns_plan* p) { k_stats<<<p->d.Ny, 256, 0, p->stream>>>(p->d); }
+void launch_stats(dns_plan* p) {
+    int EB = 1;
+    while (EB < p->d.E && EB < 32) EB <<= 1;
+    k_stats<<<dim3(p->d.Ny, (p->d.E + EB - 1) / EB), 256, 0, p->stream>>>(p->d);
+}
 
 size_t dns_ens_count(const DnsDev& d) { return 2 * ((size_t)3 * d.Ny * d.nkz + (size_t)d.Ny * d.Mz); }
 void launch_ens(dns_plan* p, int phase) {
