@@ -22,6 +22,12 @@
 
 namespace {
 
+// weight of the third RK3 stage, (F0 + 4 F1 + F2)/6, as a multiplication: a double-precision division is a
+// ~25-instruction sequence on the fp64 pipe, and the four per-element divisions of the stage-2 launch of k_ypair were 15 % of
+// its instructions (ncu, profiles/r3_kernels.md).  x * SIXTH differs from x / 6 by at most one unit in the last place.
+constexpr double SIXTH = 1.0 / 6.0;
+
+
 __device__ __forceinline__ void dmma(double (&c)[2], double a, double b) {
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
                  : "+d"(c[0]), "+d"(c[1])
@@ -170,7 +176,7 @@ __device__ void mean_body(const DnsDev& d, int stage, int derive_only, int tile,
                 const size_t gi = (size_t)j * d.E + e;
                 if (stage == 0) d.uvc0[gi] = make_double2(a, b);
                 else if (stage == 1) { const double2 s0 = d.uvc0[gi]; d.uvc0[gi] = make_double2(s0.x + 4.0 * a, s0.y + 4.0 * b); a = 2.0 * a - s0.x; b = 2.0 * b - s0.y; }
-                else { const double2 s01 = d.uvc0[gi]; a = (s01.x + a) / 6.0; b = (s01.y + b) / 6.0; }
+                else { const double2 s01 = d.uvc0[gi]; a = (s01.x + a) * SIXTH; b = (s01.y + b) * SIXTH; }
             }
             uvc[j * 8 + el] = a; wvc[j * 8 + el] = b;
         }
@@ -389,8 +395,8 @@ k_ypair(DnsDev d, const __grid_constant__ CUtensorMap tmN, const __grid_constant
                     d.G0[giB] = make_double2(ghB[k].x + 4.0 * GB.x, ghB[k].y + 4.0 * GB.y);
                 }
             } else {
-                GcA = make_double2((ghA[k].x + GA.x) / 6.0, (ghA[k].y + GA.y) / 6.0);
-                GcB = make_double2((ghB[k].x + GB.x) / 6.0, (ghB[k].y + GB.y) / 6.0);
+                GcA = make_double2((ghA[k].x + GA.x) * SIXTH, (ghA[k].y + GA.y) * SIXTH);
+                GcB = make_double2((ghB[k].x + GB.x) * SIXTH, (ghB[k].y + GB.y) * SIXTH);
             }
             const double2 rA = make_double2(2.0 * etA.x - hdt * GcA.x, 2.0 * etA.y - hdt * GcA.y);
             const double2 rB = make_double2(2.0 * etB.x - hdt * GcB.x, 2.0 * etB.y - hdt * GcB.y);
@@ -431,8 +437,8 @@ k_ypair(DnsDev d, const __grid_constant__ CUtensorMap tmN, const __grid_constant
                 if (eok && sok) d.F0[gS + 4 * nt] = make_double2(fhS[nt].x + 4.0 * FA.x, fhS[nt].y + 4.0 * FA.y);
                 if (eok && dok) d.F0[gD + 4 * nt] = make_double2(fhD[nt].x + 4.0 * FB.x, fhD[nt].y + 4.0 * FB.y);
             } else {
-                cA = make_double2((fhS[nt].x + FA.x) / 6.0, (fhS[nt].y + FA.y) / 6.0);
-                cB = make_double2((fhD[nt].x + FB.x) / 6.0, (fhD[nt].y + FB.y) / 6.0);
+                cA = make_double2((fhS[nt].x + FA.x) * SIXTH, (fhS[nt].y + FA.y) * SIXTH);
+                cB = make_double2((fhD[nt].x + FB.x) * SIXTH, (fhD[nt].y + FB.y) * SIXTH);
             }
             if (!dok) cB = cA;                              // middle row of an odd Ni: s = 2 x
             if (sok) st2(P2 + offS + 8 * nt, make_double2(-hdt * (cA.x + cB.x), -hdt * (cA.y + cB.y)));
